@@ -1,0 +1,349 @@
+#!/usr/bin/env python
+"""Benchmark of the POLFED hot path on B200 (contract: see the task statement / DESIGN.md).
+
+One "step" = one pass of the whole hot path over one block: polfed_filter_apply with a filter
+of order K_filter on BASELINE.json config 5 (spinless fermions L=26, N=13, D=10 400 600,
+nnz=275 407 888, s=32), i.e. one scaled copy + K_filter fused SpMM+Clenshaw launches.
+metric = algorithmic GB/s of that pass, bytes per fused launch = nnz*12 + 4(N+1) + 32*s*N
+(the first launch of a pass has no b_{k+2} read and is counted without it).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--order K_filter]
+  python bench.py --impl reference ...      # the CPU oracle on a bounded sample of the workload
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402  (seeded parameters only; no arithmetic of the method)
+
+METRIC = "fused_spmm_clenshaw_algorithmic_bandwidth"
+UNIT = "GB/s"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star: "B200's ~8 TB/s peak"
+FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback
+WORKLOAD_NAMES = {1: "config1_xxz_L12_s1", 2: "config2_xxz_L16_s8", 3: "config3_xxz_L20_s16",
+                  4: "config4_quantum_sun_2^20_s16", 5: "config5_fermions_L26_N13_s32"}
+
+
+def step_bytes(n: int, nnz: int, s: int, with_z: bool = True) -> int:
+    """Algorithmic bytes of one fused launch: CSR once, X, Z, V read, Y written."""
+    return nnz * 12 + 4 * (n + 1) + 8 * s * n * (4 if with_z else 3)
+
+
+def pass_bytes(n: int, nnz: int, s: int, K: int) -> int:
+    """One filter application of order K >= 1: scaled copy + (K-1) launches with Z + 1 without."""
+    return 16 * s * n + (K - 1) * step_bytes(n, nnz, s) + step_bytes(n, nnz, s, with_z=False)
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def recorded_traffic(workload: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            return json.load(fh).get(workload)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+
+    QUERY = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.lines, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}",
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def __exit__(self, *exc):
+        if self.proc is not None:
+            time.sleep(0.25)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.lines:
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for name, flag in zip(names, parts[2:6]):
+                if flag.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)),
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---- CPU oracle legs (the only places bench.py executes oracle/) -------------------------------
+
+def oracle_sample(config: int, rows_target: int, seed: int):
+    """First `rows_target` rows of the workload's matrix and full-size random blocks."""
+    from oracle import core
+    w = workloads.make_workload(config)
+    states = core.basis_states(w.n_sites, w.n_up)
+    n = int(states.shape[0])
+    m = min(n, rows_target)
+    mini = core.build_csr_rows(states, np.arange(m, dtype=np.int64), w.terms, w.dot_bits, w.dot_dense)
+    rng = np.random.Generator(np.random.PCG64(seed))
+    B1 = rng.standard_normal((n, w.s))
+    V = rng.standard_normal((m, w.s))
+    B2 = rng.standard_normal((m, w.s))
+    T = np.empty((m, w.s))
+    return w, n, mini, B1, B2, V, T
+
+
+def oracle_time_steps(mini, w, B1, B2, V, T, n_steps: int):
+    from oracle import core
+    t0 = time.perf_counter()
+    for k in range(n_steps):
+        core.clenshaw_step(mini, 0.3, 17.0, 1e-3 * (k + 1), V, B1, B2, T)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(config: int, budget_s: float = 15.0):
+    """Oracle recurrence steps (orc_clenshaw_step, as it stands) on the first rows of the workload."""
+    from oracle import core
+    rows = {1: 924, 2: 12870, 3: 184756, 4: 262144, 5: 262144}[config]
+    w, n, mini, B1, B2, V, T = oracle_sample(config, rows, seed=7000 + config)
+    oracle_time_steps(mini, w, B1, B2, V, T, 1)
+    t1 = oracle_time_steps(mini, w, B1, B2, V, T, 2) / 2
+    n_steps = int(max(3, min(200, budget_s / max(t1, 1e-6))))
+    t = oracle_time_steps(mini, w, B1, B2, V, T, n_steps) / n_steps
+    by = step_bytes(mini.n, mini.nnz, w.s)
+    return {"value": by / t / 1e9, "unit": UNIT, "cores": core.num_threads(), "kind": "oracle",
+            "sample": f"{n_steps} recurrence steps (orc_clenshaw_step) on rows [0,{mini.n}) of "
+                      f"{WORKLOAD_NAMES[config]} (nnz {mini.nnz}), full-size X block, "
+                      f"{t * 1e3:.2f} ms/step",
+            "ms_per_recurrence_step": t * 1e3}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import core
+    rows = {1: 924, 2: 12870, 3: 184756, 4: 131072, 5: 131072}[args.config]
+    w, n, mini, B1, B2, V, T = oracle_sample(args.config, rows, seed=7000 + args.config)
+    order = max(1, min(args.order, 4))
+    for _ in range(args.warmup):
+        oracle_time_steps(mini, w, B1, B2, V, T, order)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_time_steps(mini, w, B1, B2, V, T, order)
+    dt = time.perf_counter() - t0
+    by = step_bytes(mini.n, mini.nnz, w.s) * order * args.steps
+    value = by / dt / 1e9
+    sample = (f"each step = {order} oracle recurrence steps on rows [0,{mini.n}) of "
+              f"{WORKLOAD_NAMES[args.config]} (nnz {mini.nnz}), full-size X block")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES[args.config], "N": n, "s": w.s, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": core.num_threads(),
+                             "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ---- the CUDA arm -----------------------------------------------------------------------------
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2605_10191_b200 as P
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    P.lib()
+
+    # weak scaling: every rank filters its own block of its own disorder realisation (8(e))
+    w = workloads.make_workload(args.config, seed=1000 + args.config + 100 * rank)
+    t0 = time.perf_counter()
+    basis = P.polfed_build_basis(w.n_sites, w.n_up)
+    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense)
+    torch.cuda.synchronize()
+    build_s = time.perf_counter() - t0
+    n, nnz, s, K = ham.n, ham.nnz, w.s, args.order
+
+    # a, b: the middle of the spectrum with a Gershgorin-safe half-width (the bench measures
+    # throughput; parameter selection is not on the timed path).  lambda~ = 0.
+    a, b = 0.0, 80.0
+    coeffs = P.polfed_filter_coeffs(a, b, a, K_in=K)
+    gen = torch.Generator(device="cuda").manual_seed(2000 + args.config + 100 * rank)
+    V = torch.randn(n, s, dtype=torch.float64, device="cuda", generator=gen)
+    V /= V.norm(dim=0, keepdim=True)
+    W = torch.empty_like(V)
+    work = torch.empty(2 * n * s, dtype=torch.float64, device="cuda")
+
+    def one_pass():
+        P.polfed_filter_apply(ham, a, b, coeffs, s, V, W, work)
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        one_pass()
+    sync_all()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        e0.record()
+        for _ in range(args.steps):
+            one_pass()
+        e1.record()
+        sync_all()
+        ms = e0.elapsed_time(e1)
+        # dominant kernel alone: back-to-back recurrence launches, events on the launching stream
+        n_l = max(10, min(200, int(0.5e12 / max(step_bytes(n, nnz, s), 1))))
+        B1, B2 = work[: n * s].view(n, s), work[n * s:].view(n, s)
+        B1.copy_(V)
+        B2.copy_(V)
+        for _ in range(3):
+            P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, -1.0, 1e-3, B1, B2, V, B2)
+            B1, B2 = B2, B1
+        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k0.record()
+        for _ in range(n_l):
+            P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, -1.0, 1e-3, B1, B2, V, B2)
+            B1, B2 = B2, B1
+        k1.record()
+        torch.cuda.synchronize()
+        kernel_ms = k0.elapsed_time(k1) / n_l
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    total_bytes = pass_bytes(n, nnz, s, K) * args.steps * world
+    value = total_bytes / (ms * 1e-3) / 1e9
+
+    # end to end through the host-buffer entry point: H2D of V and D2H of W inside the region
+    Vh = torch.empty(n, s, dtype=torch.float64).pin_memory()
+    Wh = torch.empty(n, s, dtype=torch.float64).pin_memory()
+    Vh.copy_(V)
+    del W, work
+    torch.cuda.empty_cache()
+    e2e_steps = max(1, min(args.steps, 3))
+    P.polfed_filter_apply_host(ham, a, b, coeffs, s, Vh, Wh)
+    sync_all()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        P.polfed_filter_apply_host(ham, a, b, coeffs, s, Vh, Wh)
+    sync_all()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = pass_bytes(n, nnz, s, K) * e2e_steps * world / float(t.item()) / 1e9
+    checksum = float(Wh.double().abs().sum())
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        achieved = step_bytes(n, nnz, s) / (kernel_ms * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES[args.config], "N": n, "nnz": nnz, "s": s,
+                       "filter_order_per_step": K, "format": "csr",
+                       "bytes_per_fused_launch": step_bytes(n, nnz, s),
+                       "l2": "inputs exceed L2 (no flush)" if step_bytes(n, nnz, s) > 4 * 126e6
+                             else "working set fits L2; not flushed (the filter re-reads it by design)",
+                       "parallelism": f"replicas x{world}" if world > 1 else "single gpu",
+                       "build_seconds": build_s},
+            "filter_steps_per_s": K * args.steps * world / (ms * 1e-3),
+            "frac_of_nominal_8TBps": value / world / NOMINAL_HBM_GBS,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * s * n,
+                    "d2h_bytes_per_step": 8 * s * n, "steps": e2e_steps, "checksum": checksum},
+            "gpu_launches": args.steps * (K + 1),
+            "clocks": clocks.summary(),
+            "roofline": {"bound": "hbm", "kernel": "fused_step_kernel", "achieved": achieved,
+                         "peak": peak, "peak_source": peak_src, "unit": UNIT,
+                         "frac": achieved / peak, "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS,
+                         "launch_ms": kernel_ms, "launches_timed": n_l,
+                         "traffic": recorded_traffic(WORKLOAD_NAMES[args.config])},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(args.config)
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--order", type=int, default=64, help="filter order K per step")
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,177 @@
+/*
+ * polfed.h -- C ABI of libpolfed: the POLFED hot path on one NVIDIA B200 (sm_100a).
+ *
+ * POLFED = polynomially filtered exact diagonalisation (arxiv/paper_2605_10191).  Citations
+ * "PAPER.md:<line>" refer to the paper text this library was written from; "R<n>" to the
+ * readings listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Every function returns an int status (POLFED_OK == 0).  polfed_last_error() returns a
+ *     thread-local, NUL-terminated description of the last failure on the calling thread.
+ *     No exception crosses this boundary.
+ *   - Pointers prefixed d_ are DEVICE pointers (cudaMalloc / torch CUDA tensor data_ptr()),
+ *     h_ are HOST pointers.  Scalars are passed by value.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Unless
+ *     a function says it synchronises, work is only enqueued on that stream.
+ *   - Vector blocks are N x s, row-major ("row-interleaved": the s entries of row i are
+ *     contiguous, leading dimension s), fp64, 16-byte aligned.  s in {1,2,4,8,16,32}.
+ *   - Opaque handles (polfed_basis, polfed_ham) are owned by the library and released by
+ *     the matching *_destroy.  All blocks, outputs and workspaces are owned by the caller.
+ *   - Basis states are unsigned integers; bit i is site i (0-based); bit value 1 = spin up
+ *     (S^z = +1/2) = occupied (R12, R13).  States are ordered as ascending integers, so
+ *     rank(x) = sum_{j=1..k} C(p_j, j) with p_1 < ... < p_k the set bits of x (combinatorial
+ *     number system).  The full space (n_up < 0) has rank(x) = x.
+ *   - Random numbers never cross this boundary: model parameters arrive as arrays.
+ */
+#ifndef POLFED_H
+#define POLFED_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  POLFED_OK = 0,
+  POLFED_EINVAL = 1,     /* bad argument (NULL, unsupported s, misaligned pointer, ...) */
+  POLFED_ENOMEM = 2,     /* host or device allocation failed */
+  POLFED_ECUDA = 3,      /* a CUDA call or kernel launch failed */
+  POLFED_ERANGE = 4,     /* rescaled target outside (-1,1), b <= 0, index overflow */
+  POLFED_ENOCONV = 5,    /* eigen-solver hit max_krylov_dim before nev pairs converged */
+  POLFED_EBREAKDOWN = 6  /* rank-deficient Krylov block (R17) */
+};
+
+typedef struct polfed_basis polfed_basis;
+typedef struct polfed_ham polfed_ham;
+
+const char* polfed_last_error(void);
+/* major*10000 + minor*100 + patch */
+int polfed_version(void);
+
+/* ------------------------------------------------------------------------------------------
+ * Basis (the paper uses symmetry sectors but never says how they are
+ * enumerated, PAPER.md:510-515, 962 -- R12).
+ * ------------------------------------------------------------------------------------------ */
+
+/* Enumerate on the device all x in [0, 2^n_sites) with popcount n_up, ascending
+ * (n_up < 0: the full 2^n_sites space, no table is stored).  1 <= n_sites <= 62 and the
+ * dimension must be < 2^31.  Synchronises `stream` before returning. */
+int polfed_build_basis(int n_sites, int n_up, void* stream, polfed_basis** out);
+int polfed_basis_destroy(polfed_basis* basis);
+int polfed_basis_dim(const polfed_basis* basis, int64_t* dim);
+/* Device pointer to the dim ascending states (library-owned, valid until destroy).  For the
+ * full space the table is materialised on first call. */
+int polfed_basis_states(const polfed_basis* basis, const uint64_t** d_states);
+/* d_rank[t] = position of d_states[t] in the basis, or -1 if its popcount is not n_up or it
+ * has a bit at or above n_sites.  n >= 0 entries; enqueued on `stream`. */
+int polfed_basis_rank(const polfed_basis* basis, const uint64_t* d_states, int64_t n,
+                      int64_t* d_rank, void* stream);
+
+/* ------------------------------------------------------------------------------------------
+ * Hamiltonian assembly.  One term list covers the paper's models: XXZ chain Eq. (54)
+ * PAPER.md:858-863; quantum sun Eq. (67); the spinless-fermion chain of
+ * BASELINE.json config 5 (R15).
+ * ------------------------------------------------------------------------------------------ */
+enum {
+  POLFED_TERM_ZZ = 0,    /* amp * S^z_i S^z_j                     diagonal            */
+  POLFED_TERM_Z = 1,     /* amp * S^z_i                           diagonal, j ignored */
+  POLFED_TERM_NN = 2,    /* amp * n_i n_j                         diagonal            */
+  POLFED_TERM_N = 3,     /* amp * n_i                             diagonal, j ignored */
+  POLFED_TERM_EXCH = 4,  /* amp * (S^+_i S^-_j + h.c.)            XXZ: amp = J/2 (R13) */
+  POLFED_TERM_HOPJW = 5, /* amp * (c^+_i c_j + h.c.) with Jordan-Wigner sign
+                            (-1)^{# occupied sites strictly between i and j}           */
+  POLFED_TERM_XX = 6     /* amp * 4 S^x_i S^x_j: flips bits i and j with amplitude amp */
+};
+typedef struct {
+  int32_t i, j;
+  double amp;
+  int32_t kind;
+} polfed_term;
+
+/* Dense symmetric block acting on bits 0..n_bits-1 (the quantum-sun dot):
+ * h_dense is a HOST array, 2^n_bits x 2^n_bits row-major.  Only valid on a full-space basis. */
+typedef struct {
+  int32_t n_bits;
+  const double* h_dense;
+} polfed_dense_block;
+
+enum { POLFED_FORMAT_CSR = 0, POLFED_FORMAT_SELL = 1 /* not implemented: POLFED_EINVAL */ };
+
+/* Assemble H on the device as CSR: row_ptr int32[N+1], col int32[nnz] ascending within a
+ * row, val fp64[nnz].  The diagonal entry of every row is stored even when zero; entries
+ * that fall on the same (row, col) are summed in term order (dot block first); the diagonal
+ * is the sum of the dot-block diagonal and the diagonal terms in term order, each product
+ * and sum rounded separately (no FMA), so values are reproducible bit for bit.
+ * h_terms is a HOST array.  A term that leaves the basis gives POLFED_EINVAL.
+ * Synchronises `stream` before returning. */
+int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_terms, int n_terms,
+                             const polfed_dense_block* dot /* may be NULL */, int format,
+                             void* stream, polfed_ham** out);
+/* Wrap a caller-owned device CSR (any real symmetric matrix, columns < n, row_ptr[n] == nnz).
+ * The arrays are NOT copied and must outlive the handle. */
+int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const int32_t* d_col,
+                        const double* d_val, polfed_ham** out);
+int polfed_ham_destroy(polfed_ham* ham);
+/* Any output pointer may be NULL. */
+int polfed_ham_csr(const polfed_ham* ham, int64_t* n, int64_t* nnz, const int32_t** d_row_ptr,
+                   const int32_t** d_col, const double** d_val);
+
+/* ------------------------------------------------------------------------------------------
+ * The hot path.
+ * ------------------------------------------------------------------------------------------ */
+
+/* One fused pass, the mapping f!(Y, X) of PAPER.md:657-659 merged with the three-term update
+ * of Eq. (51) PAPER.md:427-431 and the rescaling of Eq. (31) PAPER.md:274-276:
+ *
+ *     Y[i,:] = p * sum_j H_ij X[j,:] + q * X[i,:] + r * Z[i,:] + c * V[i,:]
+ *
+ * d_Z is not read when r == 0 (may be NULL), d_V is not read when c == 0 (may be NULL).
+ * d_Y may alias d_Z or d_V (row i of Z and V is read only by the threads that write row i
+ * of Y); d_Y must not overlap d_X.  Also serves H X (p=1), Eq. (28)-(30) (KPM recurrence)
+ * and the Lanczos three-term step.  Enqueued on `stream`; allocates nothing. */
+int polfed_fused_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
+                      const double* d_X, const double* d_Z, const double* d_V, double* d_Y,
+                      void* stream);
+
+/* 2 * n * s * sizeof(double): the two auxiliary blocks of PAPER.md:431. */
+size_t polfed_filter_workspace_bytes(int64_t n, int s);
+
+/* W = sum_{k=0..K} h_coeffs[k] T_k(H~) V,  H~ = (H - a)/b, by the Clenshaw recurrence
+ * Eq. (51) PAPER.md:427-431:
+ *     b_{K+1} = b_{K+2} = 0;  b_k = h_coeffs[k] V + 2 H~ b_{k+1} - b_{k+2}  (k = K..1);
+ *     W = h_coeffs[0] V + H~ b_1 - b_2
+ * as exactly K sparse products (max(K-1,0) + 1 launches of the fused kernel, plus one scaled
+ * copy b_K = c_K V), on two rotating auxiliary blocks in d_work (pointer swap only, Fig. 5).
+ * K >= 0.  h_coeffs: K+1 HOST doubles, read before return.  d_W must not overlap d_V or
+ * d_work.  b > 0 required (POLFED_ERANGE).  Enqueued on `stream`; allocates nothing; does
+ * not synchronise. */
+int polfed_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,
+                        int s, const double* d_V, double* d_W, void* d_work, void* stream);
+
+/* Same operation on HOST blocks: allocates device blocks, copies h_V up, runs
+ * polfed_filter_apply, copies W down into h_W, frees, synchronises.  The end-to-end entry. */
+int polfed_filter_apply_host(const polfed_ham* ham, double a, double b, int K,
+                             const double* h_coeffs, int s, const double* h_V, double* h_W,
+                             void* stream);
+
+/* ------------------------------------------------------------------------------------------
+ * Filter parameters (host only).
+ * ------------------------------------------------------------------------------------------ */
+
+/* Delta-filter coefficients Eq. (32)-(33) PAPER.md:280-286 at sigma (unrescaled energy;
+ * lambda~ = (sigma - a)/b must lie in (-1,1) else POLFED_ERANGE):
+ *   c_0 = 1/chi, c_n = 2 T_n(lambda~)/chi, chi = 1 + 2 sum_{n=1..K} T_n(lambda~)^2   (R1).
+ * Order: if rho_rescaled > 0 (states per unit rescaled energy at the target), K is
+ * ceil(2.655 sqrt(1 - lambda~^2)/delta), delta = nev/(2 rho), Eq. (40), (42) PAPER.md:343-360,
+ * refined by bisection on Eq. (41) in [K/2, 2K] with cutoff Omega = sin(2.655)/2.655 (R4);
+ * otherwise K = K_in.  *K_out receives K; coeffs (capacity doubles, may be NULL to query K
+ * only) receives K+1 values; capacity < K+1 gives POLFED_EINVAL with *K_out set. */
+int polfed_filter_coeffs(double a, double b, double sigma, int nev, double rho_rescaled, int K_in,
+                         int* K_out, double* h_coeffs, int capacity);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* POLFED_H */

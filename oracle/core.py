@@ -34,6 +34,8 @@ def lib():
         L.orc_basis_rank.argtypes = [p, C.c_int64, C.c_uint64]
         L.orc_build_csr.restype = C.c_int64
         L.orc_build_csr.argtypes = [p, C.c_int64, p, C.c_int, C.c_int, p, p, p, p]
+        L.orc_build_csr_rows.restype = C.c_int64
+        L.orc_build_csr_rows.argtypes = [p, C.c_int64, p, C.c_int64, p, C.c_int, C.c_int, p, p, p, p]
         L.orc_spmm.restype = None
         L.orc_spmm.argtypes = [C.c_int64, p, p, p, C.c_int, p, p]
         L.orc_rescale.restype = None
@@ -125,6 +127,28 @@ def build_csr(states: np.ndarray, terms, dot_bits: int = 0,
     return CSR(dim, row_ptr, col, val)
 
 
+def build_csr_rows(states: np.ndarray, rows: np.ndarray, terms, dot_bits: int = 0,
+                   dot_dense: Optional[np.ndarray] = None) -> CSR:
+    """Mini-CSR holding only the matrix rows ``rows`` (columns index the full dimension);
+    ``spmm`` on it returns (H X)[rows, :].  For spot checks at full BASELINE sizes."""
+    dim = int(states.shape[0])
+    rows = np.ascontiguousarray(rows, dtype=np.int64)
+    tarr = _terms_array(terms)
+    dd = None
+    if dot_bits > 0:
+        dd = np.ascontiguousarray(dot_dense, dtype=np.float64)
+    row_ptr = np.zeros(rows.shape[0] + 1, dtype=np.int32)
+    nnz = lib().orc_build_csr_rows(_ptr(states), dim, _ptr(rows), rows.shape[0], tarr, len(terms),
+                                   dot_bits, _ptr(dd), _ptr(row_ptr), None, None)
+    if nnz < 0:
+        raise ValueError("oracle CSR build failed (a term leaves the basis?)")
+    col = np.empty(nnz, dtype=np.int32)
+    val = np.empty(nnz, dtype=np.float64)
+    lib().orc_build_csr_rows(_ptr(states), dim, _ptr(rows), rows.shape[0], tarr, len(terms),
+                             dot_bits, _ptr(dd), _ptr(row_ptr), _ptr(col), _ptr(val))
+    return CSR(int(rows.shape[0]), row_ptr, col, val)
+
+
 def hamiltonian(workload) -> Tuple[np.ndarray, CSR]:
     """(states, CSR) of a workloads.Workload."""
     states = basis_states(workload.n_sites, workload.n_up)
@@ -142,8 +166,8 @@ def _block(X: np.ndarray) -> Tuple[np.ndarray, int]:
 
 def spmm(H: CSR, X: np.ndarray) -> np.ndarray:
     X, s = _block(X)
-    assert X.shape[0] == H.n
-    Y = np.empty_like(X)
+    assert H.col.size == 0 or int(H.col.max()) < X.shape[0]
+    Y = np.empty((H.n, s), dtype=np.float64)
     lib().orc_spmm(H.n, _ptr(H.row_ptr), _ptr(H.col), _ptr(H.val), s, _ptr(X), _ptr(Y))
     return Y
 

@@ -183,6 +183,36 @@ int64_t orc_build_csr(const uint64_t *states, int64_t dim, const orc_term *terms
   return err ? -1 : (int64_t)row_ptr[dim];
 }
 
+/* The same assembly for a chosen subset of rows (spot checks at sizes where the full
+ * matrix is too slow to build on the CPU).  rows[k] in [0, dim); output row k of the
+ * mini-CSR holds matrix row rows[k], columns still index the full dimension.
+ * Two calls as above: col == NULL counts (row_ptr: int32[n_rows+1]), else fills. */
+int64_t orc_build_csr_rows(const uint64_t *states, int64_t dim, const int64_t *rows,
+                           int64_t n_rows, const orc_term *terms, int n_terms, int dot_bits,
+                           const double *dot_dense, int32_t *row_ptr, int32_t *col, double *val) {
+  int cap = n_terms + (dot_bits > 0 ? (1 << dot_bits) : 0) + 1;
+  orc_entry *e = (orc_entry *)malloc(sizeof(orc_entry) * (size_t)cap);
+  if (!e) return -1;
+  int64_t total = 0;
+  for (int64_t k = 0; k < n_rows; ++k) {
+    int n = row_entries(states, dim, rows[k], terms, n_terms, dot_bits, dot_dense, e);
+    if (n < 0) { free(e); return -1; }
+    int m = merge_entries(e, n);
+    if (!col) {
+      row_ptr[k] = (int32_t)total;
+    } else {
+      for (int q = 0; q < m; ++q) {
+        col[row_ptr[k] + q] = (int32_t)e[q].col;
+        val[row_ptr[k] + q] = e[q].val;
+      }
+    }
+    total += m;
+  }
+  if (!col) row_ptr[n_rows] = (int32_t)total;
+  free(e);
+  return total;
+}
+
 /* ---- O3: sparse matrix x block ------------------------------------------ */
 
 /* Y[i,:] = sum_{e in row i} val[e] * X[col[e],:], sequential in stored order

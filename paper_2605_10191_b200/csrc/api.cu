@@ -1,0 +1,89 @@
+// Error reporting, handle lifetime and the CSR wrapper entry points of libpolfed.
+#include <new>
+
+#include "common.cuh"
+
+namespace polfed {
+
+static thread_local std::string g_error;
+
+void set_error(const char* fmt, ...) {
+  char buf[1024];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_error = buf;
+}
+
+int fail(int code, const char* fmt, ...) {
+  char buf[1024];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_error = buf;
+  return code;
+}
+
+}  // namespace polfed
+
+using polfed::fail;
+
+extern "C" {
+
+const char* polfed_last_error(void) { return polfed::g_error.c_str(); }
+
+int polfed_version(void) { return 100; }  // 0.1.0
+
+int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const int32_t* d_col,
+                        const double* d_val, polfed_ham** out) {
+  if (!out) return fail(POLFED_EINVAL, "polfed_ham_from_csr: out is NULL");
+  *out = nullptr;
+  if (n < 0 || nnz < 0) return fail(POLFED_EINVAL, "polfed_ham_from_csr: negative size");
+  if (n >= (int64_t(1) << 31) || nnz >= (int64_t(1) << 31))
+    return fail(POLFED_ERANGE, "polfed_ham_from_csr: n and nnz must fit int32 indices");
+  if (!d_row_ptr || (nnz > 0 && (!d_col || !d_val)))
+    return fail(POLFED_EINVAL, "polfed_ham_from_csr: NULL array");
+  if (!polfed::aligned16(d_val) || (reinterpret_cast<uintptr_t>(d_col) & 3u))
+    return fail(POLFED_EINVAL, "polfed_ham_from_csr: misaligned array");
+  polfed_ham* h = new (std::nothrow) polfed_ham;
+  if (!h) return fail(POLFED_ENOMEM, "polfed_ham_from_csr: host allocation failed");
+  h->n = n;
+  h->nnz = nnz;
+  h->d_row_ptr = d_row_ptr;
+  h->d_col = d_col;
+  h->d_val = d_val;
+  h->owns = false;
+  int dev = 0, sms = 148;
+  if (cudaGetDevice(&dev) == cudaSuccess)
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  h->sm_count = sms > 0 ? sms : 148;
+  cudaGetLastError();
+  *out = h;
+  return POLFED_OK;
+}
+
+int polfed_ham_destroy(polfed_ham* ham) {
+  if (!ham) return POLFED_OK;
+  if (ham->owns) {
+    cudaFree(const_cast<int32_t*>(ham->d_row_ptr));
+    cudaFree(const_cast<int32_t*>(ham->d_col));
+    cudaFree(const_cast<double*>(ham->d_val));
+  }
+  delete ham;
+  return POLFED_OK;
+}
+
+int polfed_ham_csr(const polfed_ham* ham, int64_t* n, int64_t* nnz, const int32_t** d_row_ptr,
+                   const int32_t** d_col, const double** d_val) {
+  if (!ham) return fail(POLFED_EINVAL, "polfed_ham_csr: ham is NULL");
+  if (n) *n = ham->n;
+  if (nnz) *nnz = ham->nnz;
+  if (d_row_ptr) *d_row_ptr = ham->d_row_ptr;
+  if (d_col) *d_col = ham->d_col;
+  if (d_val) *d_val = ham->d_val;
+  return POLFED_OK;
+}
+
+}  // extern "C"

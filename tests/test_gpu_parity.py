@@ -1,0 +1,303 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Needs a B200: every test is marked gpu.
+
+Tolerances: basis states, ranks and CSR structure/values are bit-exact.  The filter output
+must satisfy relative l2 error <= 1e-9 for K <= 5000 (BASELINE.json north_star); a single
+fused step differs from the oracle only by summation order and FMA contraction (R20), so
+it is held to 1e-13 relative to the magnitude of the terms.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import workloads
+from oracle import cheb, core
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+BLOCK_SIZES = (1, 2, 4, 8, 16, 32)
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2605_10191_b200 as pkg
+    pkg.lib()                                   # fails loudly when the extension is missing
+    return pkg
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def ham_from_oracle(P, H: core.CSR):
+    return P.polfed_ham_from_csr(dev(H.row_ptr), dev(H.col), dev(H.val))
+
+
+def rel_l2(got, want):
+    return float(np.linalg.norm(got - want) / max(np.linalg.norm(want), 1e-300))
+
+
+def random_csr(n, avg, seed, empty_every=0):
+    """Random sparse symmetric-pattern-free matrix with ragged rows (some empty)."""
+    rng = np.random.default_rng(seed)
+    lens = rng.integers(0, 2 * avg + 1, size=n)
+    if empty_every:
+        lens[::empty_every] = 0
+    lens[-1] = min(n, 3 * avg + 5)               # one long row at the ragged end
+    row_ptr = np.zeros(n + 1, dtype=np.int32)
+    row_ptr[1:] = np.cumsum(lens)
+    col = np.concatenate([np.sort(rng.choice(n, size=l, replace=False)) for l in lens] +
+                         [np.zeros(0, dtype=np.int64)]).astype(np.int32)
+    val = rng.standard_normal(col.shape[0])
+    return core.CSR(n, row_ptr, col, val)
+
+
+# ---- basis: bit-exact -------------------------------------------------------------------
+
+@pytest.mark.parametrize("L,n_up", [(4, 2), (10, 5), (12, 6), (16, 8), (9, 3), (7, 0), (7, 7),
+                                    (20, 10), (13, 1), (10, -1)])
+def test_basis_states_and_ranks_bit_exact(P, L, n_up):
+    want = core.basis_states(L, n_up)
+    basis = P.polfed_build_basis(L, n_up)
+    assert basis.dim == want.shape[0]
+    got = P.polfed_basis_states(basis).cpu().numpy().view(np.uint64)
+    assert np.array_equal(got, want)
+    ranks = P.polfed_basis_rank(basis, dev(want.view(np.int64))).cpu().numpy()
+    assert np.array_equal(ranks, np.arange(want.shape[0]))
+    # states outside the sector rank to -1, as the oracle's binary search reports
+    probe = np.array([0, 1, (1 << L) - 1, 1 << L, (1 << L) + 1, 0b1011], dtype=np.uint64)
+    got_r = P.polfed_basis_rank(basis, dev(probe.view(np.int64))).cpu().numpy()
+    want_r = np.array([core.basis_rank(want, int(x)) for x in probe])
+    assert np.array_equal(got_r, want_r)
+
+
+def test_basis_rejects_bad_arguments(P):
+    for args in [(0, 0), (63, 3), (10, 11), (40, 20), (31, -1)]:
+        with pytest.raises(P.PolfedError):
+            P.polfed_build_basis(*args)
+
+
+# ---- CSR assembly: bit-exact ------------------------------------------------------------
+
+CASES = [(1, None), (2, None), (3, 14), (3, None), (4, 5), (4, 9), (4, None), (5, 8), (5, 14),
+         (5, 18)]
+
+
+@pytest.mark.parametrize("config,L_override", CASES)
+def test_hamiltonian_csr_bit_exact(P, config, L_override):
+    w = workloads.make_workload(config, L_override=L_override)
+    _, H = core.hamiltonian(w)
+    basis = P.polfed_build_basis(w.n_sites, w.n_up)
+    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense)
+    assert (ham.n, ham.nnz) == (H.n, H.nnz)
+    row_ptr, col, val = (t.cpu().numpy() for t in P.polfed_ham_csr(ham))
+    assert np.array_equal(row_ptr, H.row_ptr)
+    assert np.array_equal(col, H.col)
+    assert np.array_equal(val.view(np.uint64), H.val.view(np.uint64))   # bit for bit
+
+
+def test_duplicate_entries_are_summed_in_term_order(P):
+    L = 6
+    terms = [("EXCH", 0, 1, 0.1), ("Z", 2, 2, 0.3), ("EXCH", 1, 0, 0.2), ("EXCH", 0, 1, 1e-17),
+             ("ZZ", 0, 1, 0.7), ("NN", 3, 4, 0.5), ("N", 5, 5, -0.25), ("HOPJW", 0, 3, 0.9)]
+    st = core.basis_states(L, 3)
+    H = core.build_csr(st, terms)
+    ham = P.polfed_build_hamiltonian(P.polfed_build_basis(L, 3), terms)
+    row_ptr, col, val = (t.cpu().numpy() for t in P.polfed_ham_csr(ham))
+    assert np.array_equal(row_ptr, H.row_ptr) and np.array_equal(col, H.col)
+    assert np.array_equal(val.view(np.uint64), H.val.view(np.uint64))
+
+
+def test_term_leaving_the_sector_is_an_error(P):
+    basis = P.polfed_build_basis(6, 3)
+    with pytest.raises(P.PolfedError):
+        P.polfed_build_hamiltonian(basis, [("XX", 0, 1, 1.0)])
+    with pytest.raises(P.PolfedError):
+        P.polfed_build_hamiltonian(basis, [("Z", 6, 6, 1.0)])
+    with pytest.raises(P.PolfedError):
+        P.polfed_build_hamiltonian(basis, [("Z", 0, 0, 1.0)], fmt=P.FORMAT_SELL)
+
+
+# ---- one fused step ----------------------------------------------------------------------
+
+@pytest.mark.parametrize("s", BLOCK_SIZES)
+@pytest.mark.parametrize("n,avg,empty_every", [(1, 1, 0), (37, 3, 5), (1000, 9, 7), (4099, 27, 0)])
+def test_fused_step_matches_oracle_on_ragged_matrices(P, s, n, avg, empty_every):
+    H = random_csr(n, min(avg, n // 3 + 1), seed=11 * n + s, empty_every=empty_every)
+    rng = np.random.default_rng(5)
+    X, Z, V = (rng.standard_normal((n, s)) for _ in range(3))
+    ham = ham_from_oracle(P, H)
+    HX = core.spmm(H, X)
+    mag = core.spmm(core.CSR(H.n, H.row_ptr, H.col, np.abs(H.val)), np.abs(X))
+    for (p, q, r, c) in [(1.0, 0.0, 0.0, 0.0), (0.7, -0.3, -1.0, 0.45), (2.0, 0.1, 0.0, -1.5),
+                         (0.5, 0.0, 0.25, 0.0)]:
+        want = p * HX + q * X + r * Z + c * V
+        scale = abs(p) * mag + abs(q * X) + abs(r * Z) + abs(c * V) + 1e-300
+        Y = torch.full((n, s), float("nan"), dtype=torch.float64, device="cuda")
+        P.polfed_fused_step(ham, s, p, q, r, c, dev(X), dev(Z) if r else None,
+                            dev(V) if c else None, Y)
+        got = Y.cpu().numpy()
+        assert np.all(np.abs(got - want) <= 1e-13 * scale)
+
+
+@pytest.mark.parametrize("s", (1, 8, 32))
+def test_fused_step_in_place_over_z(P, s):
+    H = random_csr(513, 11, seed=3)
+    rng = np.random.default_rng(8)
+    X, Z, V = (rng.standard_normal((513, s)) for _ in range(3))
+    want = 0.5 * core.spmm(H, X) - 0.2 * X - Z + 0.3 * V
+    buf = dev(Z)
+    P.polfed_fused_step(ham_from_oracle(P, H), s, 0.5, -0.2, -1.0, 0.3, dev(X), buf, dev(V), buf)
+    assert rel_l2(buf.cpu().numpy(), want) < 1e-14
+
+
+def test_fused_step_rejects_bad_arguments(P):
+    H = random_csr(64, 3, seed=1)
+    ham = ham_from_oracle(P, H)
+    X = torch.zeros(64, 4, dtype=torch.float64, device="cuda")
+    Y = torch.zeros_like(X)
+    with pytest.raises(P.PolfedError):
+        P.polfed_fused_step(ham, 4, 1.0, 0.0, 0.0, 0.0, X, None, None, X)       # Y overlaps X
+    with pytest.raises(P.PolfedError):
+        P.polfed_fused_step(ham, 4, 1.0, 0.0, 1.0, 0.0, X, None, None, Y)       # r != 0, Z NULL
+    import ctypes as C
+    rc = P.lib().polfed_fused_step(C.c_void_p(ham.handle), 3, 1.0, 0.0, 0.0, 0.0,
+                                   C.c_void_p(X.data_ptr()), None, None,
+                                   C.c_void_p(Y.data_ptr()), None)                # s = 3
+    assert rc == P.binding.EINVAL and "block size" in P.polfed_last_error()
+
+
+# ---- the filter: rel l2 <= 1e-9 for K <= 5000 -----------------------------------------------
+
+def run_filter(P, ham, a, b, coeffs, V, host=False):
+    n, s = V.shape
+    if host:
+        W = np.empty_like(V)
+        P.polfed_filter_apply_host(ham, a, b, coeffs, s, V, W)
+        return W
+    W = torch.full((n, s), float("nan"), dtype=torch.float64, device="cuda")
+    work = torch.empty(2 * n * s, dtype=torch.float64, device="cuda")
+    P.polfed_filter_apply(ham, a, b, coeffs, s, dev(V), W, work)
+    return W.cpu().numpy()
+
+
+@pytest.mark.parametrize("K", [0, 1, 2, 3, 17])
+@pytest.mark.parametrize("s", (1, 4, 32))
+def test_filter_small_orders_and_edge_cases(P, K, s):
+    A, H = None, random_csr(301, 7, seed=K + 100)
+    Hs = core.CSR(H.n, H.row_ptr, H.col, H.val)
+    V = workloads.start_block(H.n, s, seed=77)
+    a, b = 0.1, 40.0                                # |spectrum| < 40 by Gershgorin-ish margin
+    coeffs = np.random.default_rng(K).standard_normal(K + 1)
+    want = core.clenshaw(Hs, a, b, coeffs, V)
+    got = run_filter(P, ham_from_oracle(P, H), a, b, coeffs, V)
+    assert rel_l2(got, want) <= 1e-12
+
+
+def bounds_and_coeffs(w, H, K=None):
+    v0 = workloads.start_block(H.n, 1, seed=3000 + w.config)[:, 0]
+    from oracle import lanczos
+    _, _, a, b = lanczos.spectrum_bounds(H, v0, m=60, margin=0.01)
+    lam = w.target if w.target_kind == "rescaled" else (w.target - a) / b
+    if K is None:
+        if w.K_fixed is not None:
+            K = w.K_fixed
+        else:
+            mu, gam = cheb.spectral_mean_width(H)
+            rho = float(cheb.gaussian_dos(a + b * lam, H.n, mu, gam)) * b   # per unit rescaled energy
+            K = cheb.order_eq42(w.nev, rho, lam)
+    return a, b, lam, K, cheb.filter_coeffs(lam, K)
+
+
+@pytest.mark.parametrize("config,L_override,K", [(1, None, None), (2, None, None), (2, None, 5000),
+                                                 (3, None, 600), (4, 11, 1000), (5, 16, 200)])
+def test_filter_matches_oracle_on_workloads(P, config, L_override, K):
+    w = workloads.make_workload(config, L_override=L_override)
+    _, H = core.hamiltonian(w)
+    a, b, lam, K, coeffs = bounds_and_coeffs(w, H, K)
+    V = workloads.start_block(H.n, w.s, seed=2000 + config, orthonormal=True)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    basis = P.polfed_build_basis(w.n_sites, w.n_up)
+    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense)
+    got = run_filter(P, ham, a, b, coeffs, V)
+    assert K <= 5000 and rel_l2(got, want) <= 1e-9
+    # the delta filter concentrates V near the target: the output is much smaller than V
+    assert np.linalg.norm(got) < np.linalg.norm(V)
+
+
+def test_filter_host_entry_point_equals_device_entry_point(P):
+    w = workloads.make_workload(2)
+    _, H = core.hamiltonian(w)
+    a, b, lam, K, coeffs = bounds_and_coeffs(w, H, K=300)
+    V = workloads.start_block(H.n, w.s, seed=2002, orthonormal=True)
+    ham = ham_from_oracle(P, H)
+    got_dev = run_filter(P, ham, a, b, coeffs, V)
+    got_host = run_filter(P, ham, a, b, coeffs, V, host=True)
+    assert np.array_equal(got_dev, got_host)
+    assert rel_l2(got_host, core.clenshaw(H, a, b, coeffs, V)) <= 1e-9
+
+
+def test_filter_rejects_bad_arguments(P):
+    H = random_csr(64, 3, seed=1)
+    ham = ham_from_oracle(P, H)
+    V = torch.zeros(64, 4, dtype=torch.float64, device="cuda")
+    W = torch.zeros_like(V)
+    work = torch.zeros(2 * 64 * 4, dtype=torch.float64, device="cuda")
+    c = np.ones(4)
+    with pytest.raises(P.PolfedError):
+        P.polfed_filter_apply(ham, 0.0, 0.0, c, 4, V, W, work)          # b = 0
+    with pytest.raises(P.PolfedError):
+        P.polfed_filter_apply(ham, 0.0, 1.0, c, 4, V, V, work)          # W overlaps V
+    with pytest.raises(P.PolfedError):
+        P.polfed_filter_apply(ham, 0.0, 1.0, c, 4, V, work[:256].view(64, 4), work)
+    with pytest.raises(ValueError):
+        P.polfed_filter_apply(ham, 0.0, 1.0, c, 4, V, W, work[:100])    # workspace too small
+
+
+# ---- full BASELINE sizes: sampled rows the oracle computes one by one ------------------------
+
+@pytest.mark.parametrize("config", [4, 5])
+def test_full_size_sampled_rows(P, config):
+    w = workloads.make_workload(config)
+    basis = P.polfed_build_basis(w.n_sites, w.n_up)
+    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense)
+    n, s = ham.n, w.s
+    states = core.basis_states(w.n_sites, w.n_up)
+    assert n == states.shape[0]
+    expected_nnz = {4: 26_214_400, 5: 275_407_888}[config]
+    assert ham.nnz == expected_nnz
+    rng = np.random.default_rng(4000 + config)
+    rows = np.unique(np.concatenate([[0, 1, n // 2, n - 2, n - 1], rng.integers(0, n, 3000)]))
+    mini = core.build_csr_rows(states, rows, w.terms, w.dot_bits, w.dot_dense)
+    row_ptr, col, val = P.polfed_ham_csr(ham)
+    row_ptr = row_ptr.cpu().numpy()
+    assert row_ptr[-1] == expected_nnz
+    lens = row_ptr[rows + 1] - row_ptr[rows]
+    assert np.array_equal(lens, np.diff(mini.row_ptr))
+    idx = np.concatenate([np.arange(row_ptr[r], row_ptr[r + 1]) for r in rows])
+    idx_d = torch.from_numpy(idx).cuda()
+    assert np.array_equal(col[idx_d].cpu().numpy(), mini.col)
+    assert np.array_equal(val[idx_d].cpu().numpy().view(np.uint64), mini.val.view(np.uint64))
+    del col, val
+    # one recurrence step b_k = c_k V + 2 H~ B1 - B2 in bench.py's launch configuration
+    gen = torch.Generator(device="cuda").manual_seed(5000 + config)
+    B1, B2, V = (torch.randn(n, s, dtype=torch.float64, device="cuda", generator=gen)
+                 for _ in range(3))
+    a, b, ck = 0.3, 17.0, 0.123
+    Y = torch.empty_like(B1)
+    P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, -1.0, ck, B1, B2, V, Y)
+    B1h = B1.cpu().numpy()
+    rows_d = torch.from_numpy(rows).cuda()
+    T = (core.spmm(mini, B1h) - a * B1h[rows]) / b                 # Eq. (31) on the sampled rows
+    want = ck * V[rows_d].cpu().numpy() + 2.0 * T - B2[rows_d].cpu().numpy()   # Eq. (51)
+    got = Y[rows_d].cpu().numpy()
+    assert np.max(np.abs(got - want)) <= 1e-12
+    # properties that hold at any size: linearity and symmetry x^T (H y) = y^T (H x)
+    HB1, HV = torch.empty_like(B1), torch.empty_like(B1)
+    P.polfed_fused_step(ham, s, 1.0, 0.0, 0.0, 0.0, B1, None, None, HB1)
+    P.polfed_fused_step(ham, s, 1.0, 0.0, 0.0, 0.0, V, None, None, HV)
+    lhs = (V * HB1).sum(0).cpu().numpy()
+    rhs = (B1 * HV).sum(0).cpu().numpy()
+    assert np.all(np.abs(lhs - rhs) <= 1e-9 * np.abs(lhs).max())
