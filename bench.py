@@ -36,14 +36,21 @@ WORKLOAD_NAMES = {1: "config1_xxz_L12_s1", 2: "config2_xxz_L16_s8", 3: "config3_
                   4: "config4_quantum_sun_2^20_s16", 5: "config5_fermions_L26_N13_s32"}
 
 
-def step_bytes(n: int, nnz: int, s: int, with_z: bool = True) -> int:
-    """Algorithmic bytes of one fused launch: CSR once, X, Z, V read, Y written."""
-    return nnz * 12 + 4 * (n + 1) + 8 * s * n * (4 if with_z else 3)
+def step_bytes(n: int, nnz: int, s: int, with_z: bool = True, with_v: bool = True) -> int:
+    """Algorithmic bytes of one fused launch: CSR once, X read, Y written, Z and V read
+    (nnz*12 + 4(N+1) + 8*s*N*4 for the full recurrence step)."""
+    return nnz * 12 + 4 * (n + 1) + 8 * s * n * (2 + int(with_z) + int(with_v))
 
 
-def pass_bytes(n: int, nnz: int, s: int, K: int) -> int:
-    """One filter application of order K >= 1: scaled copy + (K-1) launches with Z + 1 without."""
-    return 16 * s * n + (K - 1) * step_bytes(n, nnz, s) + step_bytes(n, nnz, s, with_z=False)
+def pass_bytes(n: int, nnz: int, s: int, coeffs) -> int:
+    """One filter application of order K >= 1: the scaled copy b_K = c_K V, then K fused launches.
+    The first launch has no b_{k+2}; a launch whose coefficient is exactly zero (every odd k
+    when lambda~ = 0) has no V term, and the library does not read V for it."""
+    K = len(coeffs) - 1
+    total = 16 * s * n
+    for k in range(K - 1, -1, -1):
+        total += step_bytes(n, nnz, s, with_z=(k != K - 1), with_v=(coeffs[k] != 0.0))
+    return total
 
 
 def measured_peak():
@@ -271,7 +278,7 @@ def run_cuda(args):
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms = float(t.item())
-    total_bytes = pass_bytes(n, nnz, s, K) * args.steps * world
+    total_bytes = pass_bytes(n, nnz, s, coeffs) * args.steps * world
     value = total_bytes / (ms * 1e-3) / 1e9
 
     # end to end through the host-buffer entry point: H2D of V and D2H of W inside the region
@@ -291,7 +298,7 @@ def run_cuda(args):
     t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = pass_bytes(n, nnz, s, K) * e2e_steps * world / float(t.item()) / 1e9
+    e2e_value = pass_bytes(n, nnz, s, coeffs) * e2e_steps * world / float(t.item()) / 1e9
     checksum = float(Wh.double().abs().sum())
 
     if rank == 0:
