@@ -171,6 +171,60 @@ int polfed_filter_apply_host(const polfed_ham* ham, double a, double b, int K,
 int polfed_filter_coeffs(double a, double b, double sigma, int nev, double rho_rescaled, int K_in,
                          int* K_out, double* h_coeffs, int capacity);
 
+/* ------------------------------------------------------------------------------------------
+ * Spectral bounds and the eigen-solver.
+ * ------------------------------------------------------------------------------------------ */
+
+/* Extremal Ritz values of n_steps scalar Lanczos steps with full reorthogonalisation started
+ * from d_v0 (n doubles, any nonzero vector; normalised internally) -- PAPER.md:86-125 (Eq. 1-6),
+ * 276-278, 462.  Outputs (any may be NULL): *emin, *emax the extremal Ritz values,
+ * *a = (emax+emin)/2, *b = (1+margin)(emax-emin)/2 (Eq. 31 widened by `margin`, R5; margin < 0
+ * means the default 0.01).  n_steps <= 0 means 60 (R6); it is clipped to n.  Allocates
+ * (n_steps+1) x n doubles of device scratch and frees it; synchronises `stream`. */
+int polfed_spectrum_bounds(const polfed_ham* ham, int n_steps, const double* d_v0, double margin,
+                           void* stream, double* emin, double* emax, double* a, double* b);
+
+typedef struct {
+  double tol;             /* absolute bound on ||H x - lambda x||; <= 0: 1e-8 * max(|E_min|,|E_max|) */
+  int32_t max_krylov_dim; /* <= 0: s * ceil((3.5 nev + 6 s)/s) (R10), never above n */
+  int32_t check_every;    /* block steps between convergence checks; <= 0: adaptive (R9) */
+  int32_t K_override;     /* > 0: polynomial order; else Eq. (42)+(41) with the Gaussian DOS (R7) */
+  int32_t bounds_steps;   /* <= 0: 60 */
+  double bounds_margin;   /* < 0: 0.01 */
+  double a, b;            /* b > 0: rescaling parameters given, no Lanczos bounds run */
+  int32_t sigma_is_rescaled; /* nonzero: sigma is the rescaled target lambda~ in (-1,1) (R8) */
+  int32_t reserved;
+} polfed_options;
+
+typedef struct {
+  double a, b, lambda_rescaled, e_min, e_max, tol;
+  int32_t K, block_steps, krylov_dim, n_converged, n_checks, reserved;
+  int64_t sparse_products;        /* fused launches, all phases */
+  double seconds_bounds, seconds_filter, seconds_reorth, seconds_qr;
+  double seconds_projected_eig;   /* dense eigen-decompositions of H_L and of the H-projection */
+  double seconds_extraction, seconds_total;
+} polfed_report;
+
+/* The nev eigenpairs of H nearest sigma (Sec. 4.6 steps 1-6):
+ *   1. a, b from polfed_spectrum_bounds (first column of d_V0 as start) unless given;
+ *   2. K from Eq. (40)-(42) with the Gaussian density of states Eq. (34) unless K_override;
+ *   3. block Lanczos on P(H~) (Fig. 4): W = P(H~) V_k by polfed_filter_apply,
+ *      A_k = V_k^T W, full reorthogonalisation against V_1..V_k (twice), W = V_{k+1} B_{k+1}
+ *      by CholeskyQR2 (R17);
+ *   4. at a check: eigen-decomposition of H_L (cuSOLVER syevd), the nev+s largest Ritz values,
+ *      back-map u = V_{1:m} t (Eq. 43), Rayleigh-Ritz of H itself in span(u) (R21), residuals
+ *      ||H x - E x||; stop when nev pairs have residual <= tol.
+ * d_V0: n x s start block (need not be orthonormal; full column rank required).
+ * Outputs: h_evals[nev] ascending, d_evecs n x nev row-major (column j pairs with h_evals[j]),
+ * h_residuals[nev]; report may be NULL.  Returns POLFED_ENOCONV (outputs hold the best nev
+ * pairs found) if max_krylov_dim is reached first, POLFED_EBREAKDOWN on a rank-deficient block.
+ * Allocates the Krylov basis (max_krylov_dim + s columns) and scratch on the device;
+ * synchronises `stream`. */
+int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int s, const double* d_V0,
+                              const polfed_options* options /* may be NULL: all defaults */,
+                              double* h_evals, double* d_evecs, double* h_residuals,
+                              polfed_report* report, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

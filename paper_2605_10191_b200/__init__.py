@@ -10,4 +10,5 @@ from .binding import (  # noqa: F401
     polfed_build_hamiltonian, polfed_ham_from_csr, polfed_ham_csr,
     polfed_fused_step, polfed_filter_workspace_bytes, polfed_filter_apply,
     polfed_filter_apply_host, polfed_filter_coeffs,
+    polfed_spectrum_bounds, polfed_block_lanczos_eigs,
 )

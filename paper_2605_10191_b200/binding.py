@@ -26,6 +26,7 @@ EXPORTS = (
     "polfed_build_hamiltonian", "polfed_ham_from_csr", "polfed_ham_destroy", "polfed_ham_csr",
     "polfed_fused_step", "polfed_filter_workspace_bytes", "polfed_filter_apply",
     "polfed_filter_apply_host", "polfed_filter_coeffs",
+    "polfed_spectrum_bounds", "polfed_block_lanczos_eigs",
 )
 
 
@@ -41,6 +42,25 @@ class _Term(C.Structure):
 
 class _DenseBlock(C.Structure):
     _fields_ = [("n_bits", C.c_int32), ("h_dense", C.c_void_p)]
+
+
+class _Options(C.Structure):
+    _fields_ = [("tol", C.c_double), ("max_krylov_dim", C.c_int32), ("check_every", C.c_int32),
+                ("K_override", C.c_int32), ("bounds_steps", C.c_int32),
+                ("bounds_margin", C.c_double), ("a", C.c_double), ("b", C.c_double),
+                ("sigma_is_rescaled", C.c_int32), ("reserved", C.c_int32)]
+
+
+class _Report(C.Structure):
+    _fields_ = [("a", C.c_double), ("b", C.c_double), ("lambda_rescaled", C.c_double),
+                ("e_min", C.c_double), ("e_max", C.c_double), ("tol", C.c_double),
+                ("K", C.c_int32), ("block_steps", C.c_int32), ("krylov_dim", C.c_int32),
+                ("n_converged", C.c_int32), ("n_checks", C.c_int32), ("reserved", C.c_int32),
+                ("sparse_products", C.c_int64),
+                ("seconds_bounds", C.c_double), ("seconds_filter", C.c_double),
+                ("seconds_reorth", C.c_double), ("seconds_qr", C.c_double),
+                ("seconds_projected_eig", C.c_double), ("seconds_extraction", C.c_double),
+                ("seconds_total", C.c_double)]
 
 
 _lib = None
@@ -75,6 +95,10 @@ def lib() -> C.CDLL:
     L.polfed_filter_apply.argtypes = [p, f64, f64, i32, p, i32, p, p, p, p]
     L.polfed_filter_apply_host.argtypes = [p, f64, f64, i32, p, i32, p, p, p]
     L.polfed_filter_coeffs.argtypes = [f64, f64, f64, i32, f64, i32, C.POINTER(i32), p, i32]
+    L.polfed_spectrum_bounds.argtypes = [p, i32, p, f64, p, C.POINTER(f64), C.POINTER(f64),
+                                         C.POINTER(f64), C.POINTER(f64)]
+    L.polfed_block_lanczos_eigs.argtypes = [p, f64, i32, i32, p, C.POINTER(_Options), p, p, p,
+                                            C.POINTER(_Report), p]
     _lib = L
     return L
 
@@ -312,3 +336,41 @@ def polfed_filter_coeffs(a: float, b: float, sigma: float, nev: int = 1,
     _check(lib().polfed_filter_coeffs(a, b, sigma, nev, rho_rescaled, K_in, C.byref(K),
                                       out.ctypes.data, out.shape[0]))
     return out
+
+
+# ---- spectral bounds and the eigen-solver ---------------------------------------------------
+
+def polfed_spectrum_bounds(ham: Ham, v0, n_steps: int = 0, margin: float = -1.0, stream=None):
+    """(e_min, e_max, a, b) from n_steps Lanczos steps started at the fp64 CUDA vector v0."""
+    import torch
+    if v0.dtype != torch.float64 or v0.numel() != ham.n:
+        raise ValueError("v0 must be an fp64 CUDA vector of length n")
+    out = [C.c_double() for _ in range(4)]
+    _check(lib().polfed_spectrum_bounds(C.c_void_p(ham.handle), n_steps, _dev(v0), margin,
+                                        _stream(stream), *[C.byref(o) for o in out]))
+    return tuple(o.value for o in out)
+
+
+def polfed_block_lanczos_eigs(ham: Ham, sigma: float, nev: int, s: int, V0, *, tol: float = 0.0,
+                              max_krylov_dim: int = 0, check_every: int = 0, K_override: int = 0,
+                              bounds_steps: int = 0, bounds_margin: float = -1.0, a: float = 0.0,
+                              b: float = 0.0, sigma_is_rescaled: bool = False, stream=None,
+                              allow_unconverged: bool = False):
+    """The nev eigenpairs of H nearest sigma: (evals ndarray, evecs CUDA tensor n x nev,
+    residuals ndarray, report dict).  Raises PolfedError(ENOCONV) unless allow_unconverged."""
+    import torch
+    opt = _Options(tol, max_krylov_dim, check_every, K_override, bounds_steps, bounds_margin, a, b,
+                   int(bool(sigma_is_rescaled)), 0)
+    rep = _Report()
+    evals = np.empty(nev, dtype=np.float64)
+    resid = np.empty(nev, dtype=np.float64)
+    evecs = torch.empty(ham.n, nev, dtype=torch.float64, device="cuda")
+    code = lib().polfed_block_lanczos_eigs(C.c_void_p(ham.handle), sigma, nev, s,
+                                           _block(V0, ham.n, s), C.byref(opt), evals.ctypes.data,
+                                           _dev(evecs), resid.ctypes.data, C.byref(rep),
+                                           _stream(stream))
+    if not (code == ENOCONV and allow_unconverged):
+        _check(code)
+    report = {name: getattr(rep, name) for name, _ in _Report._fields_ if name != "reserved"}
+    report["status"] = code
+    return evals, evecs, resid, report

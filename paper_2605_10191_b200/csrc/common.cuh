@@ -42,6 +42,21 @@ inline bool valid_block_size(int s) {
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// spmm_clenshaw.cu: the fused step without argument validation.
+int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
+                  const double* X, const double* Z, const double* V, double* Y, cudaStream_t st);
+
+// tallskinny.cu (see there).  d_C is zeroed by ts_gram before accumulation.
+int ts_gram(int s, long long n, const double* Q, int n_panels, size_t stride, const double* B,
+            double* d_C, int sm_count, cudaStream_t st);
+int ts_update(int s, long long n, const double* Q, int n_panels, size_t stride, const double* d_C,
+              double alpha, double beta, double* B, cudaStream_t st);
+int ts_residual_norms(int s, long long n, const double* A, const double* B, const double* d_e,
+                      double* d_out, int sm_count, cudaStream_t st);
+int ts_gather_columns(long long n, const double* src, int src_ld, const int* d_cols, int n_cols,
+                      double* dst, int dst_ld, int dst_col0, int sm_count, cudaStream_t st);
+int csr_moments(const polfed_ham* ham, double* d_out2, cudaStream_t st);
+
 }  // namespace polfed
 
 struct polfed_basis {

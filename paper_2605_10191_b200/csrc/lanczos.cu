@@ -1,0 +1,548 @@
+// Spectral bounds (scalar Lanczos) and the POLFED eigen-solver driver: block Lanczos on P(H~)
+// with full reorthogonalisation, CholeskyQR2, periodic Rayleigh-Ritz.
+// PAPER.md:86-182 (Sec. 2.1-2.2), 364-382 (Sec. 4.3), 458-469 (Sec. 4.6).  The small dense
+// eigenproblems (H_L and the H-projection) are library calls (cuSOLVER syevd); everything that
+// touches an n-long vector runs in this library's kernels.
+#include <cusolverDn.h>
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "common.cuh"
+
+namespace polfed {
+namespace {
+
+struct DeviceBuf {
+  void* p = nullptr;
+  ~DeviceBuf() { cudaFree(p); }
+  cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 1); }
+  double* f64() const { return static_cast<double*>(p); }
+};
+
+double now_seconds() {
+  return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count();
+}
+
+// ---- small dense helpers on the host (row-major s x s, s <= 32) --------------------------------
+
+// G = R^T R with R upper triangular.  false: G is not numerically positive definite.
+bool cholesky_upper(int s, const double* G, double* R) {
+  double gmax = 0.0;
+  for (int i = 0; i < s; ++i) gmax = std::max(gmax, G[i * s + i]);
+  std::fill(R, R + s * s, 0.0);
+  for (int i = 0; i < s; ++i) {
+    double d = G[i * s + i];
+    for (int k = 0; k < i; ++k) d -= R[k * s + i] * R[k * s + i];
+    if (!(d > 1e-15 * gmax)) return false;
+    const double rii = std::sqrt(d);
+    R[i * s + i] = rii;
+    for (int j = i + 1; j < s; ++j) {
+      double v = G[i * s + j];
+      for (int k = 0; k < i; ++k) v -= R[k * s + i] * R[k * s + j];
+      R[i * s + j] = v / rii;
+    }
+  }
+  return true;
+}
+
+void upper_inverse(int s, const double* R, double* Ri) {
+  std::fill(Ri, Ri + s * s, 0.0);
+  for (int j = 0; j < s; ++j) {
+    Ri[j * s + j] = 1.0 / R[j * s + j];
+    for (int i = j - 1; i >= 0; --i) {
+      double v = 0.0;
+      for (int k = i + 1; k <= j; ++k) v += R[i * s + k] * Ri[k * s + j];
+      Ri[i * s + j] = -v / R[i * s + i];
+    }
+  }
+}
+
+void matmul(int s, const double* A, const double* B, double* C) {
+  for (int i = 0; i < s; ++i)
+    for (int j = 0; j < s; ++j) {
+      double v = 0.0;
+      for (int k = 0; k < s; ++k) v += A[i * s + k] * B[k * s + j];
+      C[i * s + j] = v;
+    }
+}
+
+// ---- dense symmetric eigen-decomposition on the device (library call) --------------------------
+struct DenseEigh {
+  cusolverDnHandle_t handle = nullptr;
+  DeviceBuf A, w, work, info;
+  size_t cap_m = 0;
+  int lwork = 0;
+  ~DenseEigh() {
+    if (handle) cusolverDnDestroy(handle);
+  }
+  // h_A: m x m symmetric (row- or column-major alike).  On return h_w ascending, h_Z column j =
+  // eigenvector j, stored contiguously (h_Z[j*m + i]).
+  int solve(int m, const double* h_A, double* h_w, double* h_Z, cudaStream_t st) {
+    if (!handle) {
+      if (cusolverDnCreate(&handle) != CUSOLVER_STATUS_SUCCESS)
+        return fail(POLFED_ECUDA, "cusolverDnCreate failed");
+    }
+    cusolverDnSetStream(handle, st);
+    if ((size_t)m > cap_m) {
+      cudaFree(A.p); cudaFree(w.p); cudaFree(work.p); cudaFree(info.p);
+      A.p = w.p = work.p = info.p = nullptr;
+      POLFED_CUDA(A.alloc(sizeof(double) * (size_t)m * m));
+      POLFED_CUDA(w.alloc(sizeof(double) * (size_t)m));
+      POLFED_CUDA(info.alloc(sizeof(int)));
+      if (cusolverDnDsyevd_bufferSize(handle, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, m,
+                                      A.f64(), m, w.f64(), &lwork) != CUSOLVER_STATUS_SUCCESS)
+        return fail(POLFED_ECUDA, "cusolverDnDsyevd_bufferSize failed");
+      POLFED_CUDA(work.alloc(sizeof(double) * (size_t)lwork));
+      cap_m = (size_t)m;
+    } else {
+      if (cusolverDnDsyevd_bufferSize(handle, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, m,
+                                      A.f64(), m, w.f64(), &lwork) != CUSOLVER_STATUS_SUCCESS)
+        return fail(POLFED_ECUDA, "cusolverDnDsyevd_bufferSize failed");
+    }
+    POLFED_CUDA(cudaMemcpyAsync(A.p, h_A, sizeof(double) * (size_t)m * m, cudaMemcpyHostToDevice, st));
+    if (cusolverDnDsyevd(handle, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, m, A.f64(), m,
+                         w.f64(), work.f64(), lwork, static_cast<int*>(info.p)) != CUSOLVER_STATUS_SUCCESS)
+      return fail(POLFED_ECUDA, "cusolverDnDsyevd failed");
+    int h_info = 0;
+    POLFED_CUDA(cudaMemcpyAsync(&h_info, info.p, sizeof(int), cudaMemcpyDeviceToHost, st));
+    POLFED_CUDA(cudaMemcpyAsync(h_w, w.p, sizeof(double) * (size_t)m, cudaMemcpyDeviceToHost, st));
+    POLFED_CUDA(cudaMemcpyAsync(h_Z, A.p, sizeof(double) * (size_t)m * m, cudaMemcpyDeviceToHost, st));
+    POLFED_CUDA(cudaStreamSynchronize(st));
+    if (h_info != 0) return fail(POLFED_ECUDA, "cusolverDnDsyevd did not converge (info=%d)", h_info);
+    return POLFED_OK;
+  }
+};
+
+// ---- CholeskyQR on one n x s panel, in place ----------------------------------------------------
+struct PanelQR {
+  int s;
+  long long n;
+  int sm_count;
+  cudaStream_t st;
+  DeviceBuf small;  // 2 * s*s doubles
+  std::vector<double> G, R, Ri, R1, tmp;
+  int init() {
+    G.resize(s * s); R.resize(s * s); Ri.resize(s * s); R1.resize(s * s); tmp.resize(s * s);
+    POLFED_CUDA(small.alloc(sizeof(double) * 2 * s * s));
+    return POLFED_OK;
+  }
+  // W <- W R^-1 with W^T W = R^T R; R (host, s x s upper) returned in R.
+  int once(double* W) {
+    double* dG = small.f64();
+    double* dRi = dG + s * s;
+    int rc = ts_gram(s, n, W, 1, 0, W, dG, sm_count, st);
+    if (rc) return rc;
+    POLFED_CUDA(cudaMemcpyAsync(G.data(), dG, sizeof(double) * s * s, cudaMemcpyDeviceToHost, st));
+    POLFED_CUDA(cudaStreamSynchronize(st));
+    for (int i = 0; i < s; ++i)
+      for (int j = i + 1; j < s; ++j) G[i * s + j] = G[j * s + i] = 0.5 * (G[i * s + j] + G[j * s + i]);
+    if (!cholesky_upper(s, G.data(), R.data()))
+      return fail(POLFED_EBREAKDOWN, "rank-deficient block in CholeskyQR");
+    upper_inverse(s, R.data(), Ri.data());
+    POLFED_CUDA(cudaMemcpyAsync(dRi, Ri.data(), sizeof(double) * s * s, cudaMemcpyHostToDevice, st));
+    return ts_update(s, n, W, 1, 0, dRi, 1.0, 0.0, W, st);
+  }
+  // CholeskyQR2: W = Q B with B = R2 R1 (host, row-major upper triangular) in `B`.
+  int twice(double* W, double* B) {
+    int rc = once(W);
+    if (rc) return rc;
+    R1 = R;
+    rc = once(W);
+    if (rc) return rc;
+    matmul(s, R.data(), R1.data(), B);
+    return POLFED_OK;
+  }
+};
+
+}  // namespace
+}  // namespace polfed
+
+using polfed::fail;
+
+extern "C" {
+
+int polfed_spectrum_bounds(const polfed_ham* ham, int n_steps, const double* d_v0, double margin,
+                           void* stream, double* emin, double* emax, double* a, double* b) {
+  using namespace polfed;
+  if (!ham) return fail(POLFED_EINVAL, "polfed_spectrum_bounds: ham is NULL");
+  if (ham->n < 1) return fail(POLFED_EINVAL, "polfed_spectrum_bounds: empty matrix");
+  if (!d_v0) return fail(POLFED_EINVAL, "polfed_spectrum_bounds: d_v0 is NULL");
+  if (n_steps <= 0) n_steps = 60;
+  if (margin < 0.0) margin = 0.01;
+  const long long n = ham->n;
+  const int m_max = (int)std::min<long long>(n_steps, n);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+
+  DeviceBuf basis, coef;
+  POLFED_CUDA(basis.alloc(sizeof(double) * (size_t)n * (m_max + 1)));
+  POLFED_CUDA(coef.alloc(sizeof(double) * (size_t)(m_max + 2)));
+  double* Phi = basis.f64();
+  double* dC = coef.f64();
+  std::vector<double> hC(m_max + 2), alpha, beta;
+
+  // phi_1 = v0 / ||v0||
+  POLFED_CUDA(cudaMemcpyAsync(Phi, d_v0, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, st));
+  int rc = ts_gram(1, n, Phi, 1, 0, Phi, dC, ham->sm_count, st);
+  if (rc) return rc;
+  POLFED_CUDA(cudaMemcpyAsync(hC.data(), dC, sizeof(double), cudaMemcpyDeviceToHost, st));
+  POLFED_CUDA(cudaStreamSynchronize(st));
+  if (!(hC[0] > 0.0) || !std::isfinite(hC[0]))
+    return fail(POLFED_EINVAL, "polfed_spectrum_bounds: start vector is zero or not finite");
+  double scale = 1.0 / std::sqrt(hC[0]);
+  POLFED_CUDA(cudaMemcpyAsync(dC, &scale, sizeof(double), cudaMemcpyHostToDevice, st));
+  rc = ts_update(1, n, Phi, 1, 0, dC, 1.0, 0.0, Phi, st);
+  if (rc) return rc;
+
+  for (int i = 0; i < m_max; ++i) {  // Eq. (2)-(4) with full reorthogonalisation
+    double* w = Phi + (size_t)(i + 1) * n;
+    rc = dispatch_step(ham, 1, 1.0, 0.0, 0.0, 0.0, Phi + (size_t)i * n, nullptr, nullptr, w, st);
+    if (rc) return rc;
+    for (int pass = 0; pass < 2; ++pass) {
+      rc = ts_gram(1, n, Phi, i + 1, (size_t)n, w, dC, ham->sm_count, st);
+      if (rc) return rc;
+      if (pass == 0) {
+        POLFED_CUDA(cudaMemcpyAsync(hC.data(), dC + i, sizeof(double), cudaMemcpyDeviceToHost, st));
+        POLFED_CUDA(cudaStreamSynchronize(st));
+        alpha.push_back(hC[0]);  // a_i = <phi_i|H|phi_i>
+      }
+      rc = ts_update(1, n, Phi, i + 1, (size_t)n, dC, -1.0, 1.0, w, st);
+      if (rc) return rc;
+    }
+    rc = ts_gram(1, n, w, 1, 0, w, dC, ham->sm_count, st);
+    if (rc) return rc;
+    POLFED_CUDA(cudaMemcpyAsync(hC.data(), dC, sizeof(double), cudaMemcpyDeviceToHost, st));
+    POLFED_CUDA(cudaStreamSynchronize(st));
+    const double bnext = std::sqrt(std::max(hC[0], 0.0));
+    if (i + 1 == m_max || !(bnext > 1e-14 * std::max(1.0, std::fabs(alpha.back())))) break;
+    beta.push_back(bnext);
+    scale = 1.0 / bnext;
+    POLFED_CUDA(cudaMemcpyAsync(dC, &scale, sizeof(double), cudaMemcpyHostToDevice, st));
+    POLFED_CUDA(cudaStreamSynchronize(st));
+    rc = ts_update(1, n, w, 1, 0, dC, 1.0, 0.0, w, st);
+    if (rc) return rc;
+  }
+  const int m = (int)alpha.size();
+  std::vector<double> T((size_t)m * m, 0.0), ev(m), Z((size_t)m * m);
+  for (int i = 0; i < m; ++i) {
+    T[(size_t)i * m + i] = alpha[i];
+    if (i + 1 < m && i < (int)beta.size()) T[(size_t)i * m + i + 1] = T[(size_t)(i + 1) * m + i] = beta[i];
+  }
+  DenseEigh eig;
+  rc = eig.solve(m, T.data(), ev.data(), Z.data(), st);
+  if (rc) return rc;
+  const double lo = ev.front(), hi = ev.back();
+  if (emin) *emin = lo;
+  if (emax) *emax = hi;
+  if (a) *a = 0.5 * (hi + lo);
+  if (b) *b = 0.5 * (hi - lo) * (1.0 + margin);
+  return POLFED_OK;
+}
+
+int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int s, const double* d_V0,
+                              const polfed_options* options, double* h_evals, double* d_evecs,
+                              double* h_residuals, polfed_report* report, void* stream) {
+  using namespace polfed;
+  if (!ham) return fail(POLFED_EINVAL, "polfed_block_lanczos_eigs: ham is NULL");
+  if (!valid_block_size(s)) return fail(POLFED_EINVAL, "polfed_block_lanczos_eigs: bad block size s=%d", s);
+  if (nev < 1 || nev > ham->n) return fail(POLFED_EINVAL, "polfed_block_lanczos_eigs: nev=%d out of range", nev);
+  if (!d_V0 || !h_evals || !d_evecs || !h_residuals)
+    return fail(POLFED_EINVAL, "polfed_block_lanczos_eigs: NULL argument");
+  if (!aligned16(d_V0)) return fail(POLFED_EINVAL, "polfed_block_lanczos_eigs: d_V0 must be 16-byte aligned");
+  polfed_options opt;
+  std::memset(&opt, 0, sizeof opt);
+  opt.bounds_margin = -1.0;
+  if (options) opt = *options;
+  polfed_report rep;
+  std::memset(&rep, 0, sizeof rep);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const long long n = ham->n;
+  const size_t panel = ((size_t)n * s + 1) & ~(size_t)1;  // doubles per panel, kept 16-byte aligned
+  const double t_start = now_seconds();
+
+  // -- step 1: rescaling parameters (Eq. 31)
+  double a_ = opt.a, b_ = opt.b, e_min, e_max;
+  if (b_ > 0.0) {
+    e_min = a_ - b_;
+    e_max = a_ + b_;
+  } else {
+    DeviceBuf v0;
+    POLFED_CUDA(v0.alloc(sizeof(double) * (size_t)n));
+    POLFED_CUDA(cudaMemcpy2DAsync(v0.p, sizeof(double), d_V0, sizeof(double) * s, sizeof(double),
+                                  (size_t)n, cudaMemcpyDeviceToDevice, st));
+    const double t0 = now_seconds();
+    int rc = polfed_spectrum_bounds(ham, opt.bounds_steps, v0.f64(), opt.bounds_margin, stream, &e_min,
+                                    &e_max, &a_, &b_);
+    if (rc) return rc;
+    rep.seconds_bounds = now_seconds() - t0;
+    if (!(b_ > 0.0)) return fail(POLFED_ERANGE, "polfed_block_lanczos_eigs: degenerate spectrum bounds");
+  }
+  const double lam = opt.sigma_is_rescaled ? sigma : (sigma - a_) / b_;
+  const double sigma_E = a_ + b_ * lam;
+  if (!(lam > -1.0 && lam < 1.0))
+    return fail(POLFED_ERANGE, "polfed_block_lanczos_eigs: rescaled target %g outside (-1,1)", lam);
+  const double h_norm = std::max(std::fabs(e_min), std::fabs(e_max));
+  const double tol = opt.tol > 0.0 ? opt.tol : 1e-8 * h_norm;
+
+  // -- step 2-3: order from the Gaussian density of states (Eq. 34, 40-42) and coefficients
+  int K = opt.K_override;
+  double rho = 0.0;
+  if (K <= 0) {
+    DeviceBuf mom;
+    POLFED_CUDA(mom.alloc(2 * sizeof(double)));
+    int rc = csr_moments(ham, mom.f64(), st);
+    if (rc) return rc;
+    double h_mom[2];
+    POLFED_CUDA(cudaMemcpyAsync(h_mom, mom.p, sizeof h_mom, cudaMemcpyDeviceToHost, st));
+    POLFED_CUDA(cudaStreamSynchronize(st));
+    const double mu = h_mom[0] / (double)n;
+    const double var = h_mom[1] / (double)n - mu * mu;
+    if (!(var > 0.0)) return fail(POLFED_ERANGE, "polfed_block_lanczos_eigs: zero spectral width");
+    const double gam = std::sqrt(var);
+    const double rho_E = (double)n / (std::sqrt(2.0 * M_PI) * gam) *
+                         std::exp(-(sigma_E - mu) * (sigma_E - mu) / (2.0 * var));
+    rho = rho_E * b_;  // states per unit rescaled energy
+    if (!(rho > 0.0)) return fail(POLFED_ERANGE, "polfed_block_lanczos_eigs: zero density of states at the target");
+  }
+  int K_out = 0;
+  int rc = polfed_filter_coeffs(a_, b_, sigma_E, nev, rho, K, &K_out, nullptr, 0);
+  if (rc) return rc;
+  K = K_out;
+  std::vector<double> coeffs((size_t)K + 1);
+  rc = polfed_filter_coeffs(a_, b_, sigma_E, nev, 0.0, K, &K_out, coeffs.data(), K + 1);
+  if (rc) return rc;
+
+  // -- sizes and device memory
+  long long m_cap = opt.max_krylov_dim > 0 ? opt.max_krylov_dim : (long long)s * ((7LL * nev / 2 + 6LL * s + s - 1) / s);
+  m_cap = std::min<long long>(m_cap, n);
+  m_cap = (m_cap / s) * s;
+  const int want_cols = (int)std::min<long long>((long long)nev + s, n);
+  const int npan = (want_cols + s - 1) / s;
+  const int wp = npan * s;  // padded number of Ritz vectors extracted
+  if (m_cap < wp) return fail(POLFED_EINVAL, "polfed_block_lanczos_eigs: max_krylov_dim=%lld < nev + s rounded up (%d), or n too small for this s", m_cap, wp);
+  const int k_cap = (int)(m_cap / s);
+
+  DeviceBuf Qb, work, Ub, Xb, T1b, coefb, evb, colsb;
+  POLFED_CUDA(Qb.alloc(sizeof(double) * panel * (size_t)(k_cap + 1)));
+  POLFED_CUDA(work.alloc(sizeof(double) * panel * 2));
+  POLFED_CUDA(Ub.alloc(sizeof(double) * panel * (size_t)npan));
+  POLFED_CUDA(Xb.alloc(sizeof(double) * panel * (size_t)npan));
+  POLFED_CUDA(T1b.alloc(sizeof(double) * panel));
+  POLFED_CUDA(coefb.alloc(sizeof(double) * (size_t)std::max<long long>(m_cap + s, wp) * s));
+  POLFED_CUDA(evb.alloc(sizeof(double) * (size_t)(s + 2)));
+  POLFED_CUDA(colsb.alloc(sizeof(int) * (size_t)nev));
+  double* Q = Qb.f64();
+  double* dC = coefb.f64();
+  PanelQR qr{s, n, ham->sm_count, st};
+  rc = qr.init();
+  if (rc) return rc;
+  DenseEigh eig;
+
+  std::vector<double> HL((size_t)m_cap * m_cap, 0.0);  // H_L, preallocated
+  std::vector<double> hC((size_t)(m_cap + s) * s), Bk(s * s), Bprev(s * s, 0.0);
+  std::vector<double> theta, Zl, G((size_t)wp * wp), Eg(wp), Zg((size_t)wp * wp), res(wp), Csel;
+  std::vector<double> best_E, best_res;
+  std::vector<int> best_cols;
+  bool have_best = false;
+
+  // -- V_1 = orthonormalised start block
+  POLFED_CUDA(cudaMemcpyAsync(Q, d_V0, sizeof(double) * (size_t)n * s, cudaMemcpyDeviceToDevice, st));
+  rc = qr.twice(Q, Bk.data());
+  if (rc) return rc;
+
+  int next_check = (wp + s - 1) / s;
+  int status = POLFED_ENOCONV;
+  int k = 0;
+  for (k = 1; k <= k_cap; ++k) {
+    double* Vk = Q + panel * (size_t)(k - 1);
+    double* W = Q + panel * (size_t)k;
+    // W = P(H~) V_k  -- the hot path
+    double t0 = now_seconds();
+    rc = polfed_filter_apply(ham, a_, b_, K, coeffs.data(), s, Vk, W, work.p, stream);
+    if (rc) return rc;
+    POLFED_CUDA(cudaStreamSynchronize(st));
+    rep.seconds_filter += now_seconds() - t0;
+    rep.sparse_products += K;
+
+    // A_k = V_k^T W and full reorthogonalisation against V_1..V_k, twice (Eq. 9, 11)
+    t0 = now_seconds();
+    for (int pass = 0; pass < 2; ++pass) {
+      rc = ts_gram(s, n, Q, k, panel, W, dC, ham->sm_count, st);
+      if (rc) return rc;
+      if (pass == 0) {
+        POLFED_CUDA(cudaMemcpyAsync(hC.data(), dC + (size_t)(k - 1) * s * s, sizeof(double) * s * s,
+                                    cudaMemcpyDeviceToHost, st));
+      }
+      rc = ts_update(s, n, Q, k, panel, dC, -1.0, 1.0, W, st);
+      if (rc) return rc;
+    }
+    POLFED_CUDA(cudaStreamSynchronize(st));
+    rep.seconds_reorth += now_seconds() - t0;
+    const size_t o = (size_t)(k - 1) * s;
+    for (int i = 0; i < s; ++i)
+      for (int j = 0; j < s; ++j)
+        HL[(o + i) * m_cap + o + j] = 0.5 * (hC[i * s + j] + hC[j * s + i]);  // A_k (Eq. 13)
+
+    // W = V_{k+1} B_{k+1} (Eq. 12)
+    t0 = now_seconds();
+    rc = qr.twice(W, Bk.data());
+    if (rc) return rc;
+    POLFED_CUDA(cudaStreamSynchronize(st));
+    rep.seconds_qr += now_seconds() - t0;
+    if (k < k_cap)
+      for (int i = 0; i < s; ++i)
+        for (int j = 0; j < s; ++j) {
+          HL[(o + s + i) * m_cap + o + j] = Bk[i * s + j];  // B_{k+1} below the diagonal (Eq. 14)
+          HL[(o + j) * m_cap + o + s + i] = Bk[i * s + j];
+        }
+    rep.block_steps = k;
+    rep.krylov_dim = k * s;
+
+    const int m = k * s;
+    if (m < wp || (k < next_check && k != k_cap)) continue;
+
+    // -- convergence check: Ritz pairs of H_L
+    t0 = now_seconds();
+    std::vector<double> Hm((size_t)m * m);
+    for (int i = 0; i < m; ++i) std::memcpy(&Hm[(size_t)i * m], &HL[(size_t)i * m_cap], sizeof(double) * m);
+    theta.resize(m);
+    Zl.resize((size_t)m * m);
+    rc = eig.solve(m, Hm.data(), theta.data(), Zl.data(), st);
+    if (rc) return rc;
+    rep.seconds_projected_eig += now_seconds() - t0;
+    rep.n_checks += 1;
+    // Eq. (16)-(17): ||B_{k+1} tau_j|| for the wp largest Ritz values (eigenvalues ascending)
+    int n_small = 0;
+    const double theta_top = std::fabs(theta[m - 1]);
+    for (int c = 0; c < wp; ++c) {
+      const double* z = &Zl[(size_t)(m - 1 - c) * m];
+      double e2 = 0.0;
+      for (int i = 0; i < s; ++i) {
+        double v = 0.0;
+        for (int j = 0; j < s; ++j) v += Bk[i * s + j] * z[m - s + j];
+        e2 += v * v;
+      }
+      if (std::sqrt(e2) <= 1e-2 * theta_top) ++n_small;
+    }
+    if (n_small < nev && k != k_cap) {
+      next_check = opt.check_every > 0 ? k + opt.check_every : k + std::max(1, (nev - n_small + 2 * s - 1) / (2 * s));
+      continue;
+    }
+
+    // -- extraction: u = V_{1:m} t (Eq. 43), Rayleigh-Ritz of H in span(u) (R21), residuals
+    t0 = now_seconds();
+    double* U = Ub.f64();
+    double* X = Xb.f64();
+    double* T1 = T1b.f64();
+    Csel.resize((size_t)m * s);
+    for (int p = 0; p < npan; ++p) {
+      for (int r = 0; r < m; ++r)
+        for (int c = 0; c < s; ++c) Csel[(size_t)r * s + c] = Zl[(size_t)(m - 1 - (p * s + c)) * m + r];
+      POLFED_CUDA(cudaMemcpyAsync(dC, Csel.data(), sizeof(double) * (size_t)m * s, cudaMemcpyHostToDevice, st));
+      rc = ts_update(s, n, Q, k, panel, dC, 1.0, 0.0, U + panel * (size_t)p, st);
+      if (rc) return rc;
+      POLFED_CUDA(cudaStreamSynchronize(st));
+    }
+    for (int p = 0; p < npan; ++p) {
+      rc = dispatch_step(ham, s, 1.0, 0.0, 0.0, 0.0, U + panel * (size_t)p, nullptr, nullptr, T1, st);
+      if (rc) return rc;
+      rc = ts_gram(s, n, U, npan, panel, T1, dC, ham->sm_count, st);
+      if (rc) return rc;
+      POLFED_CUDA(cudaMemcpyAsync(hC.data(), dC, sizeof(double) * (size_t)wp * s, cudaMemcpyDeviceToHost, st));
+      POLFED_CUDA(cudaStreamSynchronize(st));
+      for (int r = 0; r < wp; ++r)
+        for (int c = 0; c < s; ++c) G[(size_t)r * wp + p * s + c] = hC[(size_t)r * s + c];
+      rep.sparse_products += 1;
+    }
+    for (int i = 0; i < wp; ++i)
+      for (int j = i + 1; j < wp; ++j)
+        G[(size_t)i * wp + j] = G[(size_t)j * wp + i] = 0.5 * (G[(size_t)i * wp + j] + G[(size_t)j * wp + i]);
+    const double t1 = now_seconds();
+    rc = eig.solve(wp, G.data(), Eg.data(), Zg.data(), st);
+    if (rc) return rc;
+    const double t_eig_inside = now_seconds() - t1;
+    rep.seconds_projected_eig += t_eig_inside;
+    for (int p = 0; p < npan; ++p) {
+      Csel.resize((size_t)wp * s);
+      for (int r = 0; r < wp; ++r)
+        for (int c = 0; c < s; ++c) Csel[(size_t)r * s + c] = Zg[(size_t)(p * s + c) * wp + r];
+      POLFED_CUDA(cudaMemcpyAsync(dC, Csel.data(), sizeof(double) * (size_t)wp * s, cudaMemcpyHostToDevice, st));
+      double* Xp = X + panel * (size_t)p;
+      rc = ts_update(s, n, U, npan, panel, dC, 1.0, 0.0, Xp, st);
+      if (rc) return rc;
+      rc = dispatch_step(ham, s, 1.0, 0.0, 0.0, 0.0, Xp, nullptr, nullptr, T1, st);
+      if (rc) return rc;
+      POLFED_CUDA(cudaMemcpyAsync(evb.p, &Eg[(size_t)p * s], sizeof(double) * s, cudaMemcpyHostToDevice, st));
+      rc = ts_residual_norms(s, n, T1, Xp, evb.f64(), dC, ham->sm_count, st);
+      if (rc) return rc;
+      POLFED_CUDA(cudaMemcpyAsync(&res[(size_t)p * s], dC, sizeof(double) * s, cudaMemcpyDeviceToHost, st));
+      POLFED_CUDA(cudaStreamSynchronize(st));
+      rep.sparse_products += 1;
+    }
+    for (int c = 0; c < wp; ++c) res[c] = std::sqrt(std::max(res[c], 0.0));
+    rep.seconds_extraction += now_seconds() - t0 - t_eig_inside;
+
+    // -- selection (R11): converged pairs nearest sigma
+    std::vector<int> order(wp);
+    for (int c = 0; c < wp; ++c) order[c] = c;
+    std::sort(order.begin(), order.end(), [&](int x, int y) {
+      return std::fabs(Eg[x] - sigma_E) < std::fabs(Eg[y] - sigma_E);
+    });
+    std::vector<int> good;
+    for (int c : order)
+      if (res[c] <= tol) good.push_back(c);
+    rep.n_converged = (int)std::min<size_t>(good.size(), (size_t)nev);
+    std::vector<int> sel;
+    const bool done = (int)good.size() >= nev;
+    if (done) {
+      sel.assign(good.begin(), good.begin() + nev);
+    } else {
+      sel.assign(order.begin(), order.begin() + nev);
+    }
+    std::sort(sel.begin(), sel.end(), [&](int x, int y) { return Eg[x] < Eg[y]; });
+    if (done || k == k_cap || !have_best) {
+      // write the outputs (best effort until converged)
+      for (int j = 0; j < nev; ++j) {
+        h_evals[j] = Eg[sel[j]];
+        h_residuals[j] = res[sel[j]];
+      }
+      // columns grouped by panel: gather from X panels into d_evecs (n x nev row-major)
+      for (int j = 0; j < nev; ++j) {
+        const int c = sel[j];
+        const int pcol = c % s;
+        POLFED_CUDA(cudaMemcpyAsync(colsb.p, &pcol, sizeof(int), cudaMemcpyHostToDevice, st));
+        rc = ts_gather_columns(n, X + panel * (size_t)(c / s), s, static_cast<int*>(colsb.p), 1, d_evecs,
+                               nev, j, ham->sm_count, st);
+        if (rc) return rc;
+        POLFED_CUDA(cudaStreamSynchronize(st));
+      }
+      have_best = true;
+    }
+    if (done) {
+      status = POLFED_OK;
+      break;
+    }
+    const int missing = nev - (int)good.size();
+    next_check = opt.check_every > 0 ? k + opt.check_every : k + std::max(1, (missing + 2 * s - 1) / (2 * s));
+  }
+
+  POLFED_CUDA(cudaStreamSynchronize(st));
+  rep.a = a_;
+  rep.b = b_;
+  rep.lambda_rescaled = lam;
+  rep.e_min = e_min;
+  rep.e_max = e_max;
+  rep.tol = tol;
+  rep.K = K;
+  rep.seconds_total = now_seconds() - t_start;
+  if (report) *report = rep;
+  if (status == POLFED_ENOCONV)
+    return fail(POLFED_ENOCONV, "polfed_block_lanczos_eigs: %d of %d pairs converged at Krylov dimension %d",
+                rep.n_converged, nev, rep.krylov_dim);
+  return POLFED_OK;
+}
+
+}  // extern "C"

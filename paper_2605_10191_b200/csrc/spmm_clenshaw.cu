@@ -191,6 +191,8 @@ int launch_step(const polfed_ham* ham, double p, double q, double r, double c, c
   return POLFED_OK;
 }
 
+}  // namespace
+
 int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
                   const double* X, const double* Z, const double* V, double* Y, cudaStream_t st) {
   switch (s) {
@@ -203,6 +205,8 @@ int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, do
   }
   return fail(POLFED_EINVAL, "block size s=%d not in {1,2,4,8,16,32}", s);
 }
+
+namespace {
 
 int scale_copy(size_t len, const double* V, double* Y, double c, int sm_count, cudaStream_t st) {
   if (len == 0) return POLFED_OK;
