@@ -71,6 +71,27 @@ def recorded_traffic(workload: str):
         return None
 
 
+def replica_seed(config: int, rank: int) -> int:
+    """Weak scaling over replicas: rank r filters its own disorder realisation."""
+    return 1000 + config + 100 * rank
+
+
+def reduce_max(value: float, device="cpu") -> float:
+    """MAX over ranks of a per-rank time (identity when torch.distributed is not initialised)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gbs(bytes_per_rank: int, world: int, seconds_max: float) -> float:
+    """Aggregate throughput: what all ranks processed / the slowest rank's time."""
+    return bytes_per_rank * world / seconds_max / 1e9
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
 
@@ -220,7 +241,7 @@ def run_cuda(args):
     P.lib()
 
     # weak scaling: every rank filters its own block of its own disorder realisation (8(e))
-    w = workloads.make_workload(args.config, seed=1000 + args.config + 100 * rank)
+    w = workloads.make_workload(args.config, seed=replica_seed(args.config, rank))
     t0 = time.perf_counter()
     basis = P.polfed_build_basis(w.n_sites, w.n_up)
     ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense)
@@ -274,12 +295,8 @@ def run_cuda(args):
         k1.record()
         torch.cuda.synchronize()
         kernel_ms = k0.elapsed_time(k1) / n_l
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    total_bytes = pass_bytes(n, nnz, s, coeffs) * args.steps * world
-    value = total_bytes / (ms * 1e-3) / 1e9
+    ms = reduce_max(ms, "cuda")
+    value = whole_job_gbs(pass_bytes(n, nnz, s, coeffs) * args.steps, world, ms * 1e-3)
 
     # end to end through the host-buffer entry point: H2D of V and D2H of W inside the region
     Vh = torch.empty(n, s, dtype=torch.float64).pin_memory()
@@ -295,10 +312,8 @@ def run_cuda(args):
         P.polfed_filter_apply_host(ham, a, b, coeffs, s, Vh, Wh)
     sync_all()
     e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = pass_bytes(n, nnz, s, coeffs) * e2e_steps * world / float(t.item()) / 1e9
+    e2e_value = whole_job_gbs(pass_bytes(n, nnz, s, coeffs) * e2e_steps, world,
+                              reduce_max(e2e_s, "cuda"))
     checksum = float(Wh.double().abs().sum())
 
     if rank == 0:
@@ -327,6 +342,10 @@ def run_cuda(args):
                          "launch_ms": kernel_ms, "launches_timed": n_l,
                          "traffic": recorded_traffic(WORKLOAD_NAMES[args.config])},
         }
+        if world == 1 and args.eigs:
+            del Vh, Wh, V
+            torch.cuda.empty_cache()
+            line["seconds_to_nev"] = [time_to_nev(P, int(c)) for c in args.eigs.split(",") if c]
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(args.config)
         print(json.dumps(line))
@@ -334,6 +353,31 @@ def run_cuda(args):
         dist.barrier()
         dist.destroy_process_group()
     return 0
+
+
+def time_to_nev(P, config: int):
+    """Second half of BASELINE.json's metric: wall seconds of polfed_block_lanczos_eigs (bounds,
+    order rule, block Lanczos on P(H~), Rayleigh-Ritz, residuals) for the workload's nev pairs."""
+    import torch
+    w = workloads.make_workload(config)
+    basis = P.polfed_build_basis(w.n_sites, w.n_up)
+    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense)
+    V0 = torch.from_numpy(workloads.start_block(ham.n, w.s, seed=2000 + config)).cuda()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    evals, evecs, resid, rep = P.polfed_block_lanczos_eigs(
+        ham, w.target, w.nev, w.s, V0, sigma_is_rescaled=(w.target_kind == "rescaled"),
+        K_override=(w.K_fixed or 0), allow_unconverged=True)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    hnorm = max(abs(rep["e_min"]), abs(rep["e_max"]))
+    return {"workload": WORKLOAD_NAMES[config], "nev": w.nev, "seconds": wall,
+            "converged": rep["status"] == 0, "K": rep["K"], "block_steps": rep["block_steps"],
+            "krylov_dim": rep["krylov_dim"], "sparse_products": rep["sparse_products"],
+            "max_residual_over_normH": float(resid.max()) / hnorm,
+            "seconds_filter": rep["seconds_filter"], "seconds_reorth": rep["seconds_reorth"],
+            "seconds_qr": rep["seconds_qr"], "seconds_projected_eig": rep["seconds_projected_eig"],
+            "seconds_extraction": rep["seconds_extraction"], "seconds_bounds": rep["seconds_bounds"]}
 
 
 def main():
@@ -345,6 +389,8 @@ def main():
     ap.add_argument("--order", type=int, default=64, help="filter order K per step")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--eigs", default="1,2,3",
+                    help="configs whose full eigen-solve is timed at N=1 ('' to skip; 4 takes minutes)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":

@@ -186,7 +186,7 @@ int polfed_spectrum_bounds(const polfed_ham* ham, int n_steps, const double* d_v
 
 typedef struct {
   double tol;             /* absolute bound on ||H x - lambda x||; <= 0: 1e-8 * max(|E_min|,|E_max|) */
-  int32_t max_krylov_dim; /* <= 0: s * ceil((3.5 nev + 6 s)/s) (R10), never above n */
+  int32_t max_krylov_dim; /* <= 0: 5 nev + 8 s rounded up to a multiple of s (R10), capped by n and by free memory */
   int32_t check_every;    /* block steps between convergence checks; <= 0: adaptive (R9) */
   int32_t K_override;     /* > 0: polynomial order; else Eq. (42)+(41) with the Gaussian DOS (R7) */
   int32_t bounds_steps;   /* <= 0: 60 */

@@ -316,12 +316,22 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
   if (rc) return rc;
 
   // -- sizes and device memory
-  long long m_cap = opt.max_krylov_dim > 0 ? opt.max_krylov_dim : (long long)s * ((7LL * nev / 2 + 6LL * s + s - 1) / s);
-  m_cap = std::min<long long>(m_cap, n);
-  m_cap = (m_cap / s) * s;
   const int want_cols = (int)std::min<long long>((long long)nev + s, n);
   const int npan = (want_cols + s - 1) / s;
   const int wp = npan * s;  // padded number of Ritz vectors extracted
+  long long m_cap = opt.max_krylov_dim;
+  if (m_cap <= 0) {
+    // R10: 5 nev + 8 s columns, but never more than fits in 85 % of the free device memory
+    m_cap = 5LL * nev + 8LL * s;
+    size_t free_b = 0, total_b = 0;
+    POLFED_CUDA(cudaMemGetInfo(&free_b, &total_b));
+    const double panel_bytes = (double)panel * sizeof(double);
+    const long long fit = (long long)(0.85 * (double)free_b / panel_bytes) - (2LL * npan + 4);
+    m_cap = std::min<long long>(m_cap, std::max<long long>(fit, npan) * s);
+  }
+  m_cap = std::min<long long>(m_cap, n);
+  m_cap = ((m_cap + s - 1) / s) * s;
+  if (m_cap > n) m_cap -= s;
   if (m_cap < wp) return fail(POLFED_EINVAL, "polfed_block_lanczos_eigs: max_krylov_dim=%lld < nev + s rounded up (%d), or n too small for this s", m_cap, wp);
   const int k_cap = (int)(m_cap / s);
 
