@@ -97,7 +97,11 @@ typedef struct {
   const double* h_dense;
 } polfed_dense_block;
 
-enum { POLFED_FORMAT_CSR = 0, POLFED_FORMAT_SELL = 1 /* not implemented: POLFED_EINVAL */ };
+enum {
+  POLFED_FORMAT_CSR = 0,
+  POLFED_FORMAT_SELL = 1, /* not implemented: POLFED_EINVAL */
+  POLFED_FORMAT_TILED = 2 /* CSR plus the tiled structured format below */
+};
 
 /* Assemble H on the device as CSR: row_ptr int32[N+1], col int32[nnz] ascending within a
  * row, val fp64[nnz].  The diagonal entry of every row is stored even when zero; entries
@@ -109,6 +113,20 @@ enum { POLFED_FORMAT_CSR = 0, POLFED_FORMAT_SELL = 1 /* not implemented: POLFED_
 int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_terms, int n_terms,
                              const polfed_dense_block* dot /* may be NULL */, int format,
                              void* stream, polfed_ham** out);
+/* POLFED_FORMAT_TILED (the paper's "optimized mapping" for constant off-diagonal values,
+ * PAPER.md:625-651, 779; north_star's structured alternative): besides the CSR, the handle gets
+ * a tile table for chains whose hops conserve the particle number.  Rows that share their top
+ * n_sites - m bits (m = ceil(n_sites/2)) are one tile; hops among the low m sites stay inside it
+ * and are stored once per particle-number class as neighbour index + sign, grouped by the at
+ * most 4 distinct |amp| values; hops among the high sites are tile-local in the site-reversed
+ * row order; the diagonal and the few hops across the cut stay a small CSR.
+ * polfed_filter_apply then runs the recurrence as sweeps that alternate between the two row
+ * orders with the tile held in shared memory (same result up to rounding order).
+ * Requirements (else POLFED_EINVAL): fixed-n_up basis, 4 <= n_sites <= 26, no dense block,
+ * off-diagonal terms of kind EXCH or HOPJW only, at most 4 distinct |amp| and 24 hops per state
+ * inside a tile.  Used by polfed_filter_apply for s in {16, 32}; every other entry point uses
+ * the CSR. */
+
 /* Wrap a caller-owned device CSR (any real symmetric matrix, columns < n, row_ptr[n] == nnz).
  * The arrays are NOT copied and must outlive the handle. */
 int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const int32_t* d_col,
@@ -137,6 +155,10 @@ int polfed_fused_step(const polfed_ham* ham, int s, double p, double q, double r
 
 /* 2 * n * s * sizeof(double): the two auxiliary blocks of PAPER.md:431. */
 size_t polfed_filter_workspace_bytes(int64_t n, int s);
+/* Workspace polfed_filter_apply needs for this handle: the value above for a CSR handle; for a
+ * POLFED_FORMAT_TILED handle and s in {16, 32}: 6 blocks (two b/partial pairs, V in both row
+ * orders) plus a per-CTA tile scratch. */
+size_t polfed_filter_workspace_bytes_ham(const polfed_ham* ham, int s);
 
 /* W = sum_{k=0..K} h_coeffs[k] T_k(H~) V,  H~ = (H - a)/b, by the Clenshaw recurrence
  * Eq. (51) PAPER.md:427-431:
@@ -144,9 +166,11 @@ size_t polfed_filter_workspace_bytes(int64_t n, int s);
  *     W = h_coeffs[0] V + H~ b_1 - b_2
  * as exactly K sparse products (max(K-1,0) + 1 launches of the fused kernel, plus one scaled
  * copy b_K = c_K V), on two rotating auxiliary blocks in d_work (pointer swap only, Fig. 5).
- * K >= 0.  h_coeffs: K+1 HOST doubles, read before return.  d_W must not overlap d_V or
- * d_work.  b > 0 required (POLFED_ERANGE).  Enqueued on `stream`; allocates nothing; does
- * not synchronise. */
+ * K >= 0.  h_coeffs: K+1 HOST doubles, read before return.  d_work holds
+ * polfed_filter_workspace_bytes_ham(ham, s) bytes.  d_W must not overlap d_V or d_work.
+ * b > 0 required (POLFED_ERANGE).  Enqueued on `stream`; allocates nothing; does not
+ * synchronise.  On a POLFED_FORMAT_TILED handle with s in {16, 32} the same recurrence runs as
+ * K + 1 launches of the tiled sweep kernel (see POLFED_FORMAT_TILED). */
 int polfed_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,
                         int s, const double* d_V, double* d_W, void* d_work, void* stream);
 

@@ -17,14 +17,15 @@ LIB_PATH = os.path.join(_HERE, "libpolfed.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ERANGE, ENOCONV, EBREAKDOWN = range(7)
 TERM_KINDS = {"ZZ": 0, "Z": 1, "NN": 2, "N": 3, "EXCH": 4, "HOPJW": 5, "XX": 6}
-FORMAT_CSR, FORMAT_SELL = 0, 1
+FORMAT_CSR, FORMAT_SELL, FORMAT_TILED = 0, 1, 2
 
 EXPORTS = (
     "polfed_last_error", "polfed_version",
     "polfed_build_basis", "polfed_basis_destroy", "polfed_basis_dim", "polfed_basis_states",
     "polfed_basis_rank",
     "polfed_build_hamiltonian", "polfed_ham_from_csr", "polfed_ham_destroy", "polfed_ham_csr",
-    "polfed_fused_step", "polfed_filter_workspace_bytes", "polfed_filter_apply",
+    "polfed_fused_step", "polfed_filter_workspace_bytes", "polfed_filter_workspace_bytes_ham",
+    "polfed_filter_apply",
     "polfed_filter_apply_host", "polfed_filter_coeffs",
     "polfed_spectrum_bounds", "polfed_block_lanczos_eigs",
 )
@@ -92,6 +93,8 @@ def lib() -> C.CDLL:
     L.polfed_fused_step.argtypes = [p, i32, f64, f64, f64, f64, p, p, p, p, p]
     L.polfed_filter_workspace_bytes.restype = C.c_size_t
     L.polfed_filter_workspace_bytes.argtypes = [i64, i32]
+    L.polfed_filter_workspace_bytes_ham.restype = C.c_size_t
+    L.polfed_filter_workspace_bytes_ham.argtypes = [p, i32]
     L.polfed_filter_apply.argtypes = [p, f64, f64, i32, p, i32, p, p, p, p]
     L.polfed_filter_apply_host.argtypes = [p, f64, f64, i32, p, i32, p, p, p]
     L.polfed_filter_coeffs.argtypes = [f64, f64, f64, i32, f64, i32, C.POINTER(i32), p, i32]
@@ -295,13 +298,18 @@ def polfed_filter_workspace_bytes(n: int, s: int) -> int:
     return int(lib().polfed_filter_workspace_bytes(n, s))
 
 
+def polfed_filter_workspace_bytes_ham(ham: Ham, s: int) -> int:
+    return int(lib().polfed_filter_workspace_bytes_ham(C.c_void_p(ham.handle), s))
+
+
 def polfed_filter_apply(ham: Ham, a: float, b: float, coeffs: np.ndarray, s: int, V, W, work,
                         stream=None) -> None:
     """W = sum_k coeffs[k] T_k((H-a)/b) V; K = len(coeffs) - 1; work holds
-    polfed_filter_workspace_bytes(n, s) bytes."""
+    polfed_filter_workspace_bytes_ham(ham, s) bytes."""
     c = np.ascontiguousarray(coeffs, dtype=np.float64)
     K = c.shape[0] - 1
-    if work is not None and work.numel() * work.element_size() < polfed_filter_workspace_bytes(ham.n, s):
+    if work is not None and \
+            work.numel() * work.element_size() < polfed_filter_workspace_bytes_ham(ham, s):
         raise ValueError("workspace too small")
     _check(lib().polfed_filter_apply(C.c_void_p(ham.handle), a, b, K, c.ctypes.data, s,
                                      _block(V, ham.n, s), _block(W, ham.n, s), _dev(work),

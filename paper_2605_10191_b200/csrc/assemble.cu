@@ -19,11 +19,6 @@ namespace {
 
 constexpr int kMaxRowEntries = 128;
 
-struct DevTerm {
-  int32_t i, j, kind, pad;
-  double amp;
-};
-
 struct ToI64 {
   __host__ __device__ long long operator()(int v) const { return (long long)v; }
 };
@@ -169,52 +164,16 @@ struct Scratch {  // frees device temporaries on every exit path
 };
 
 }  // namespace
-}  // namespace polfed
 
-using polfed::fail;
-
-extern "C" int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_terms,
-                                        int n_terms, const polfed_dense_block* dot, int format,
-                                        void* stream, polfed_ham** out) {
-  using namespace polfed;
-  if (!out) return fail(POLFED_EINVAL, "polfed_build_hamiltonian: out is NULL");
-  *out = nullptr;
-  if (!basis) return fail(POLFED_EINVAL, "polfed_build_hamiltonian: basis is NULL");
-  if (format != POLFED_FORMAT_CSR)
-    return fail(POLFED_EINVAL, "polfed_build_hamiltonian: only POLFED_FORMAT_CSR is implemented");
-  if (n_terms < 0 || (n_terms > 0 && !h_terms))
-    return fail(POLFED_EINVAL, "polfed_build_hamiltonian: bad term list");
-  int dot_bits = 0;
-  if (dot && dot->n_bits > 0) {
-    dot_bits = dot->n_bits;
-    if (basis->n_up >= 0)
-      return fail(POLFED_EINVAL, "polfed_build_hamiltonian: a dense block needs the full space");
-    if (dot_bits > 6 || dot_bits > basis->n_sites || !dot->h_dense)
-      return fail(POLFED_EINVAL, "polfed_build_hamiltonian: bad dense block");
-  }
-  std::vector<DevTerm> terms((size_t)n_terms);
-  int n_offdiag = dot_bits ? (1 << dot_bits) - 1 : 0;
-  for (int t = 0; t < n_terms; ++t) {
-    const polfed_term& s = h_terms[t];
-    if (s.kind < POLFED_TERM_ZZ || s.kind > POLFED_TERM_XX)
-      return fail(POLFED_EINVAL, "polfed_build_hamiltonian: term %d has unknown kind %d", t, s.kind);
-    const bool one_site = (s.kind == POLFED_TERM_Z || s.kind == POLFED_TERM_N);
-    const int j = one_site ? s.i : s.j;
-    if (s.i < 0 || s.i >= basis->n_sites || j < 0 || j >= basis->n_sites)
-      return fail(POLFED_EINVAL, "polfed_build_hamiltonian: term %d acts outside the lattice", t);
-    if (s.kind >= POLFED_TERM_EXCH) {
-      if (s.i == j)
-        return fail(POLFED_EINVAL, "polfed_build_hamiltonian: term %d needs two distinct sites", t);
-      ++n_offdiag;
-    }
-    terms[t] = DevTerm{s.i, j, s.kind, 0, s.amp};
-  }
-  if (n_offdiag + 1 > kMaxRowEntries)
-    return fail(POLFED_EINVAL, "polfed_build_hamiltonian: more than %d entries per row",
-                kMaxRowEntries);
+// CSR of the term list over the basis (the work of polfed_build_hamiltonian; also used for the
+// diagonal + cross-cut parts of the tiled format, tiled_plan.cu).  Arrays are cudaMalloc'ed;
+// the caller owns them.  Synchronises `st`.
+int assemble_csr(const polfed_basis* basis, const std::vector<DevTerm>& terms, int dot_bits,
+                 const double* h_dot, cudaStream_t st, int32_t** out_row_ptr, int32_t** out_col,
+                 double** out_val, long long* out_nnz) {
+  const int n_terms = (int)terms.size();
   int rc = ensure_binomials();
   if (rc) return rc;
-  cudaStream_t st = static_cast<cudaStream_t>(stream);
   const int64_t dim = basis->dim;
 
   Scratch tmp;
@@ -233,15 +192,14 @@ extern "C" int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_
   if (dot_bits) {
     const size_t dd = (size_t)1 << dot_bits;
     POLFED_CUDA(tmp.alloc(&d_dot, sizeof(double) * dd * dd));
-    POLFED_CUDA(cudaMemcpyAsync(d_dot, dot->h_dense, sizeof(double) * dd * dd,
-                                cudaMemcpyHostToDevice, st));
+    POLFED_CUDA(cudaMemcpyAsync(d_dot, h_dot, sizeof(double) * dd * dd, cudaMemcpyHostToDevice, st));
   }
   POLFED_CUDA(cudaMemsetAsync(d_flag, 0, sizeof(int), st));
   POLFED_CUDA(cudaMemsetAsync(d_counts, 0, sizeof(int32_t) * (size_t)(dim + 1), st));
 
   int32_t* d_row_ptr = nullptr;
   POLFED_CUDA(cudaMalloc(&d_row_ptr, sizeof(int32_t) * (size_t)(dim + 1)));
-  struct Guard {  // releases the result arrays unless ownership moved to the handle
+  struct Guard {  // releases the result arrays unless ownership moved to the caller
     int32_t* a = nullptr;
     int32_t* b = nullptr;
     double* c = nullptr;
@@ -292,12 +250,80 @@ extern "C" int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_
     POLFED_LAUNCH_CHECK("assemble_kernel<fill>");
   }
   POLFED_CUDA(cudaStreamSynchronize(st));
-
-  polfed_ham* h = nullptr;
-  rc = polfed_ham_from_csr(dim, total, d_row_ptr, d_col, d_val, &h);
-  if (rc) return rc;
-  h->owns = true;
   guard.armed = false;
+  *out_row_ptr = d_row_ptr;
+  *out_col = d_col;
+  *out_val = d_val;
+  *out_nnz = total;
+  return POLFED_OK;
+}
+
+}  // namespace polfed
+
+using polfed::fail;
+
+extern "C" int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_terms,
+                                        int n_terms, const polfed_dense_block* dot, int format,
+                                        void* stream, polfed_ham** out) {
+  using namespace polfed;
+  if (!out) return fail(POLFED_EINVAL, "polfed_build_hamiltonian: out is NULL");
+  *out = nullptr;
+  if (!basis) return fail(POLFED_EINVAL, "polfed_build_hamiltonian: basis is NULL");
+  if (format != POLFED_FORMAT_CSR && format != POLFED_FORMAT_TILED)
+    return fail(POLFED_EINVAL,
+                "polfed_build_hamiltonian: format must be POLFED_FORMAT_CSR or POLFED_FORMAT_TILED");
+  if (n_terms < 0 || (n_terms > 0 && !h_terms))
+    return fail(POLFED_EINVAL, "polfed_build_hamiltonian: bad term list");
+  int dot_bits = 0;
+  if (dot && dot->n_bits > 0) {
+    dot_bits = dot->n_bits;
+    if (basis->n_up >= 0)
+      return fail(POLFED_EINVAL, "polfed_build_hamiltonian: a dense block needs the full space");
+    if (dot_bits > 6 || dot_bits > basis->n_sites || !dot->h_dense)
+      return fail(POLFED_EINVAL, "polfed_build_hamiltonian: bad dense block");
+  }
+  std::vector<DevTerm> terms((size_t)n_terms);
+  int n_offdiag = dot_bits ? (1 << dot_bits) - 1 : 0;
+  for (int t = 0; t < n_terms; ++t) {
+    const polfed_term& s = h_terms[t];
+    if (s.kind < POLFED_TERM_ZZ || s.kind > POLFED_TERM_XX)
+      return fail(POLFED_EINVAL, "polfed_build_hamiltonian: term %d has unknown kind %d", t, s.kind);
+    const bool one_site = (s.kind == POLFED_TERM_Z || s.kind == POLFED_TERM_N);
+    const int j = one_site ? s.i : s.j;
+    if (s.i < 0 || s.i >= basis->n_sites || j < 0 || j >= basis->n_sites)
+      return fail(POLFED_EINVAL, "polfed_build_hamiltonian: term %d acts outside the lattice", t);
+    if (s.kind >= POLFED_TERM_EXCH) {
+      if (s.i == j)
+        return fail(POLFED_EINVAL, "polfed_build_hamiltonian: term %d needs two distinct sites", t);
+      ++n_offdiag;
+    }
+    terms[t] = DevTerm{s.i, j, s.kind, 0, s.amp};
+  }
+  if (n_offdiag + 1 > kMaxRowEntries)
+    return fail(POLFED_EINVAL, "polfed_build_hamiltonian: more than %d entries per row",
+                kMaxRowEntries);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  int32_t* d_row_ptr = nullptr;
+  int32_t* d_col = nullptr;
+  double* d_val = nullptr;
+  long long total = 0;
+  int rc = assemble_csr(basis, terms, dot_bits, dot_bits ? dot->h_dense : nullptr, st, &d_row_ptr,
+                        &d_col, &d_val, &total);
+  if (rc) return rc;
+  polfed_ham* h = nullptr;
+  rc = polfed_ham_from_csr(basis->dim, total, d_row_ptr, d_col, d_val, &h);
+  if (rc) {
+    cudaFree(d_row_ptr); cudaFree(d_col); cudaFree(d_val);
+    return rc;
+  }
+  h->owns = true;
+  if (format == POLFED_FORMAT_TILED) {
+    rc = build_tiled_plan(basis, terms, st, &h->tiled);
+    if (rc) {
+      polfed_ham_destroy(h);
+      return rc;
+    }
+  }
   *out = h;
   return POLFED_OK;
 }

@@ -7,6 +7,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <string>
+#include <vector>
 
 #include "polfed.h"
 
@@ -42,6 +43,27 @@ inline bool valid_block_size(int s) {
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// One term of the Hamiltonian as the device kernels read it (polfed_term with j filled in).
+struct DevTerm {
+  int32_t i, j, kind, pad;
+  double amp;
+};
+
+struct TiledPlan;  // tiled.cuh
+
+// assemble.cu: CSR of a term list over a basis; arrays cudaMalloc'ed, owned by the caller.
+int assemble_csr(const polfed_basis* basis, const std::vector<DevTerm>& terms, int dot_bits,
+                 const double* h_dot, cudaStream_t st, int32_t** out_row_ptr, int32_t** out_col,
+                 double** out_val, long long* out_nnz);
+// tiled_plan.cu / tiled_sweep.cu: the tiled (matrix-free inside a tile) format, see tiled.cuh.
+int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& terms, cudaStream_t st,
+                     TiledPlan** out);
+void destroy_tiled_plan(TiledPlan* plan);
+bool tiled_supports(const polfed_ham* ham, int s);
+size_t tiled_workspace_bytes(const polfed_ham* ham, int s);
+int tiled_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,
+                       int s, const double* d_V, double* d_W, void* d_work, cudaStream_t st);
+
 // spmm_clenshaw.cu: the fused step without argument validation.
 int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
                   const double* X, const double* Z, const double* V, double* Y, cudaStream_t st);
@@ -74,4 +96,5 @@ struct polfed_ham {
   const double* d_val = nullptr;
   bool owns = false;  // arrays allocated by polfed_build_hamiltonian
   int sm_count = 148;
+  polfed::TiledPlan* tiled = nullptr;  // POLFED_FORMAT_TILED only (owned)
 };

@@ -337,7 +337,7 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
 
   DeviceBuf Qb, work, Ub, Xb, T1b, coefb, evb, colsb;
   POLFED_CUDA(Qb.alloc(sizeof(double) * panel * (size_t)(k_cap + 1)));
-  POLFED_CUDA(work.alloc(sizeof(double) * panel * 2));
+  POLFED_CUDA(work.alloc(polfed_filter_workspace_bytes_ham(ham, s)));
   POLFED_CUDA(Ub.alloc(sizeof(double) * panel * (size_t)npan));
   POLFED_CUDA(Xb.alloc(sizeof(double) * panel * (size_t)npan));
   POLFED_CUDA(T1b.alloc(sizeof(double) * panel));

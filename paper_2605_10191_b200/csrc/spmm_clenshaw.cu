@@ -259,6 +259,12 @@ size_t polfed_filter_workspace_bytes(int64_t n, int s) {
   return (size_t)2 * (size_t)n * (size_t)s * sizeof(double);
 }
 
+size_t polfed_filter_workspace_bytes_ham(const polfed_ham* ham, int s) {
+  if (!ham || s < 1) return 0;
+  if (polfed::tiled_supports(ham, s)) return polfed::tiled_workspace_bytes(ham, s);
+  return polfed_filter_workspace_bytes(ham->n, s);
+}
+
 int polfed_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,
                         int s, const double* d_V, double* d_W, void* d_work, void* stream) {
   if (!ham) return fail(POLFED_EINVAL, "polfed_filter_apply: ham is NULL");
@@ -274,14 +280,17 @@ int polfed_filter_apply(const polfed_ham* ham, double a, double b, int K, const 
     return fail(POLFED_EINVAL, "polfed_filter_apply: blocks must be 16-byte aligned");
   const size_t len = (size_t)ham->n * s;
   const size_t bytes = len * sizeof(double);
+  const size_t work_bytes = polfed_filter_workspace_bytes_ham(ham, s);
   if (polfed::overlap(d_V, bytes, d_W, bytes) ||
-      (K >= 1 && (polfed::overlap(d_work, 2 * bytes, d_W, bytes) ||
-                  polfed::overlap(d_work, 2 * bytes, d_V, bytes))))
+      (K >= 1 && (polfed::overlap(d_work, work_bytes, d_W, bytes) ||
+                  polfed::overlap(d_work, work_bytes, d_V, bytes))))
     return fail(POLFED_EINVAL, "polfed_filter_apply: V, W and work must not overlap");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
 
   if (K == 0)  // W = c_0 V
     return polfed::scale_copy(len, d_V, d_W, h_coeffs[0], ham->sm_count, st);
+  if (polfed::tiled_supports(ham, s))  // the alternating-layout pipeline of tiled.cuh
+    return polfed::tiled_filter_apply(ham, a, b, K, h_coeffs, s, d_V, d_W, d_work, st);
 
   double* cur = static_cast<double*>(d_work);  // b_{k+1}
   double* old = cur + len;                     // b_{k+2}, overwritten by b_k
@@ -312,8 +321,8 @@ int polfed_filter_apply_host(const polfed_ham* ham, double a, double b, int K,
   if (!h_V || !h_W) return fail(POLFED_EINVAL, "polfed_filter_apply_host: NULL block");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const size_t bytes = (size_t)ham->n * s * sizeof(double);
-  double* d_all = nullptr;  // V | W | work(2)
-  POLFED_CUDA(cudaMalloc(&d_all, 4 * bytes));
+  double* d_all = nullptr;  // V | W | work
+  POLFED_CUDA(cudaMalloc(&d_all, 2 * bytes + polfed_filter_workspace_bytes_ham(ham, s)));
   const size_t len = bytes / sizeof(double);
   double* d_V = d_all;
   double* d_W = d_all + len;

@@ -1,0 +1,134 @@
+"""Parity of the tiled format (POLFED_FORMAT_TILED: alternating-layout Clenshaw pipeline with the
+tile in shared memory, include/polfed.h) against the CPU oracle's textbook Clenshaw on the same
+seeded inputs.  The tiled path must give the filter output of Eq. (51) PAPER.md:427-431 within
+rel l2 <= 1e-9 (north_star); it differs from the oracle only in summation order.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import workloads
+from oracle import cheb, core
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2605_10191_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def rel_l2(got, want):
+    return float(np.linalg.norm(got - want) / max(np.linalg.norm(want), 1e-300))
+
+
+def tiled_filter(P, ham, a, b, coeffs, V):
+    n, s = V.shape
+    need = P.polfed_filter_workspace_bytes_ham(ham, s)
+    assert need > P.polfed_filter_workspace_bytes(n, s)          # the tiled path is in use
+    work = torch.full((need // 8,), float("nan"), dtype=torch.float64, device="cuda")
+    W = torch.full((n, s), float("nan"), dtype=torch.float64, device="cuda")
+    P.polfed_filter_apply(ham, a, b, coeffs, s, dev(V), W, work)
+    return W.cpu().numpy()
+
+
+def build(P, n_sites, n_up, terms, fmt=None):
+    basis = P.polfed_build_basis(n_sites, n_up)
+    return P.polfed_build_hamiltonian(basis, terms, fmt=P.FORMAT_TILED if fmt is None else fmt)
+
+
+def gershgorin(H):
+    rad = np.zeros(H.n)
+    np.add.at(rad, np.repeat(np.arange(H.n), np.diff(H.row_ptr)), np.abs(H.val))
+    return float(rad.max())
+
+
+FERMION = [(8, 4), (12, 6), (12, 3), (13, 6), (14, 9), (16, 8)]
+
+
+@pytest.mark.parametrize("K", [1, 2, 3, 4, 9, 40])
+@pytest.mark.parametrize("s", (16, 32))
+@pytest.mark.parametrize("L,n_up", FERMION)
+def test_tiled_filter_random_coefficients(P, L, n_up, s, K):
+    rng = np.random.default_rng(100 * L + n_up)
+    terms = workloads.fermion_terms(L, 1.0, 0.5, 1.0, rng.uniform(-2, 2, L))
+    st = core.basis_states(L, n_up)
+    H = core.build_csr(st, terms)
+    V = workloads.start_block(H.n, s, seed=7 * L + K)
+    a, b = 0.37, 1.05 * gershgorin(H)
+    coeffs = np.random.default_rng(K).standard_normal(K + 1)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    got = tiled_filter(P, build(P, L, n_up, terms), a, b, coeffs, V)
+    assert rel_l2(got, want) <= 1e-12
+
+
+@pytest.mark.parametrize("config,L_override,K", [(5, 16, 200), (5, 18, 1000), (3, 14, 600),
+                                                 (3, 16, None)])
+def test_tiled_filter_matches_oracle_on_workloads(P, config, L_override, K):
+    w = workloads.make_workload(config, L_override=L_override)
+    _, H = core.hamiltonian(w)
+    from oracle import lanczos
+    v0 = workloads.start_block(H.n, 1, seed=3000 + config)[:, 0]
+    _, _, a, b = lanczos.spectrum_bounds(H, v0, m=60, margin=0.01)
+    lam = w.target
+    if K is None:
+        mu, gam = cheb.spectral_mean_width(H)
+        K = cheb.order_eq42(w.nev, float(cheb.gaussian_dos(a + b * lam, H.n, mu, gam)) * b, lam)
+    coeffs = cheb.filter_coeffs(lam, K)
+    V = workloads.start_block(H.n, w.s, seed=2000 + config, orthonormal=True)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    got = tiled_filter(P, build(P, w.n_sites, w.n_up, w.terms), a, b, coeffs, V)
+    assert K <= 5000 and rel_l2(got, want) <= 1e-9
+
+
+def test_tiled_handles_signs_long_hops_and_several_amplitudes(P):
+    """Negative amplitudes, a hop across the cut, duplicate bonds, periodic closure, four
+    distinct |amp| inside a tile."""
+    L, n_up, s = 12, 5, 16
+    terms = [("HOPJW", 0, 1, -0.7), ("HOPJW", 1, 3, 0.7), ("EXCH", 2, 5, 0.3), ("HOPJW", 4, 0, 1.1),
+             ("EXCH", 1, 2, 0.25), ("HOPJW", 0, 1, 0.7),
+             ("HOPJW", 5, 6, 0.9), ("HOPJW", 3, 9, -0.4), ("EXCH", 11, 0, 0.6),
+             ("HOPJW", 7, 10, 0.8), ("EXCH", 6, 11, -0.8), ("HOPJW", 8, 9, 0.2),
+             ("NN", 2, 7, 0.5), ("N", 11, 11, -1.5), ("ZZ", 0, 6, 0.9), ("Z", 3, 3, 0.4)]
+    H = core.build_csr(core.basis_states(L, n_up), terms)
+    V = workloads.start_block(H.n, s, seed=5)
+    coeffs = np.random.default_rng(1).standard_normal(12)
+    a, b = -0.2, 1.1 * gershgorin(H)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    got = tiled_filter(P, build(P, L, n_up, terms), a, b, coeffs, V)
+    assert rel_l2(got, want) <= 1e-12
+
+
+def test_tiled_ineligible_requests_fail_loudly(P):
+    five = [("HOPJW", i, i + 1, 1.0 + 0.1 * i) for i in range(5)]
+    for n_sites, n_up, terms in [(8, -1, [("XX", 0, 1, 1.0)]),            # full space
+                                 (12, 6, five),                             # 5 amplitudes in a tile
+                                 (3, 1, [("EXCH", 0, 1, 1.0)]),             # too short
+                                 (28, 1, [("EXCH", 0, 1, 1.0)])]:           # tile would not fit smem
+        basis = P.polfed_build_basis(n_sites, n_up)
+        with pytest.raises(P.PolfedError):
+            P.polfed_build_hamiltonian(basis, terms, fmt=P.FORMAT_TILED)
+
+
+def test_tiled_handle_still_serves_csr_entry_points(P):
+    w = workloads.make_workload(5, L_override=12)
+    _, H = core.hamiltonian(w)
+    ham = build(P, w.n_sites, w.n_up, w.terms)
+    row_ptr, col, val = (t.cpu().numpy() for t in P.polfed_ham_csr(ham))
+    assert np.array_equal(col, H.col) and np.array_equal(val, H.val)
+    # block sizes the tiled path does not cover fall back to the CSR kernel
+    V = workloads.start_block(H.n, 4, seed=1)
+    assert P.polfed_filter_workspace_bytes_ham(ham, 4) == P.polfed_filter_workspace_bytes(H.n, 4)
+    coeffs = np.random.default_rng(2).standard_normal(6)
+    W = torch.empty(H.n, 4, dtype=torch.float64, device="cuda")
+    work = torch.empty(2 * H.n * 4, dtype=torch.float64, device="cuda")
+    P.polfed_filter_apply(ham, 0.0, 20.0, coeffs, 4, dev(V), W, work)
+    assert rel_l2(W.cpu().numpy(), core.clenshaw(H, 0.0, 20.0, coeffs, V)) <= 1e-12
