@@ -46,7 +46,12 @@ int upload(T** d, const std::vector<T>& h) {
 }
 
 // Records of one layout: `low` holds the tile-local hops with sites already in this layout's
-// numbering (all < m).
+// numbering (all < m).  Class k (k particles on the low m sites) owns records
+// class_off[k] .. class_off[k+1]; they are sorted by falling degree so that the rows a warp
+// works on together have (nearly) the same number of neighbours.  Record = 16 words:
+//   word 0      row index inside the tile (bits 0-10) | degree (bits 16-20)
+//   words 1-12  24 entries of 16 bits: neighbour row (bits 0-10) | amplitude class (bits 11-12)
+//               | sign (bit 15); unused entries point at the zero row (index = rows of the class)
 int build_records(int m, const std::vector<DevTerm>& low, TiledLayout* lay,
                   std::vector<uint32_t>* rec, const std::vector<int>& class_off) {
   lay->n_coef = 0;
@@ -66,12 +71,10 @@ int build_records(int m, const std::vector<DevTerm>& low, TiledLayout* lay,
     cls[t] = c;
   }
   rec->assign((size_t)(1u << m) * kTileRecWords, 0u);
-  std::vector<uint32_t> ent[kTileMaxCoef];
+  std::vector<std::vector<uint16_t>> ent((size_t)1 << m);  // by class_off[k] + class_rank(l)
   for (uint32_t l = 0; l < (1u << m); ++l) {
     const int k = __builtin_popcount(l);
-    const size_t row = (size_t)class_off[k] + class_rank(l);
-    for (auto& e : ent) e.clear();
-    int deg = 0;
+    std::vector<uint16_t>& e = ent[(size_t)class_off[k] + class_rank(l)];
     for (size_t t = 0; t < low.size(); ++t) {
       if (cls[t] < 0) continue;
       const int i = low[t].i, j = low[t].j;
@@ -83,19 +86,26 @@ int build_records(int m, const std::vector<DevTerm>& low, TiledLayout* lay,
         const uint32_t between = ((1u << hi) - 1u) & ~((2u << lo) - 1u);
         sign ^= (uint32_t)__builtin_popcount(l & between) & 1u;
       }
-      ent[cls[t]].push_back(class_rank(l2) | (sign << 15));
-      ++deg;
+      e.push_back((uint16_t)(class_rank(l2) | ((uint32_t)cls[t] << 11) | (sign << 15)));
     }
-    if (deg > kTileMaxDeg)
+    if ((int)e.size() > kTileMaxDeg)
       return fail(POLFED_EINVAL, "tiled format: more than %d hops inside a tile for one state",
                   kTileMaxDeg);
-    uint32_t* w = rec->data() + row * kTileRecWords;
-    int at = 0;
-    for (int c = 0; c < kTileMaxCoef; ++c) {
-      w[0] |= (uint32_t)ent[c].size() << (8 * c);
-      for (uint32_t e : ent[c]) {
-        w[1 + (at >> 1)] |= e << (16 * (at & 1));
-        ++at;
+  }
+  for (int k = 0; k <= m; ++k) {
+    const int n_k = class_off[k + 1] - class_off[k];
+    std::vector<int> order(n_k);
+    for (int r = 0; r < n_k; ++r) order[r] = r;
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) {
+      return ent[(size_t)class_off[k] + x].size() > ent[(size_t)class_off[k] + y].size();
+    });
+    for (int t = 0; t < n_k; ++t) {
+      const std::vector<uint16_t>& e = ent[(size_t)class_off[k] + order[t]];
+      uint32_t* w = rec->data() + ((size_t)class_off[k] + t) * kTileRecWords;
+      w[0] = (uint32_t)order[t] | ((uint32_t)e.size() << 16);
+      for (int j = 0; j < kTileMaxDeg; ++j) {
+        const uint32_t v = j < (int)e.size() ? e[j] : (uint32_t)n_k;  // zero row
+        w[1 + (j >> 1)] |= v << (16 * (j & 1));
       }
     }
   }

@@ -8,8 +8,6 @@
 namespace polfed {
 namespace {
 
-constexpr int kGroups = kTileThreads / 8;  // 8 lanes x 16 bytes = one 128-byte panel row
-
 enum { MODE_STEP = 0, MODE_INIT = 1, MODE_LAST = 2 };
 
 struct SweepArgs {
@@ -17,7 +15,7 @@ struct SweepArgs {
   int n_tiles, n_panels, max_tile_rows;
   const int32_t* tile_row0;
   const int32_t* tile_rec0;
-  const uint2* records;  // 8 x uint2 per class row
+  const uint32_t* records;  // kTileRecWords words per class row
   const int32_t* dm_row_ptr;
   const int32_t* dm_col;
   const double* dm_val;
@@ -84,50 +82,70 @@ __device__ __forceinline__ void tile_load(void* dst, const void* src, unsigned b
   }
 }
 
-// sum over the in-tile neighbours of one class row: coef * sign * xs[neighbour]; the loop count is
-// warp-uniform (max_deg), rows with fewer entries are predicated off.
+// Thread mapping: 4 lanes own one 128-byte panel row (two 16-byte chunks each), a warp works on
+// 8 rows at a time.  Even row slots read chunk q first and chunk q+4 second, odd slots the other
+// way round, so that the two rows of a quarter-warp always hit disjoint shared-memory banks.
+
+// One in-tile neighbour: entry in bits 16..31 of t = row (11 bits) | class (2) | sign (bit 31).
 template <int NC>
-__device__ __forceinline__ double2 tile_hops(const double2* __restrict__ xs, uint2 rec2,
-                                             uint32_t header, int max_deg, int l,
-                                             const double (&coef)[kTileMaxCoef]) {
-  const int n0 = header & 0xff, n1 = n0 + ((header >> 8) & 0xff), n2 = n1 + ((header >> 16) & 0xff);
-  const int deg = n2 + (header >> 24);
-  double2 acc = make_double2(0.0, 0.0);
-  for (int j = 0; j < max_deg; ++j) {
-    const int w = 1 + (j >> 1);
-    const uint32_t word = __shfl_sync(0xffffffffu, (w & 1) ? rec2.y : rec2.x, w >> 1, 8);
-    if (j < deg) {
-      const uint32_t e = (word >> ((j & 1) * 16)) & 0xffffu;
-      double cf = coef[0];
-      if (NC > 1 && j >= n0) cf = coef[1];
-      if (NC > 2 && j >= n1) cf = coef[2];
-      if (NC > 3 && j >= n2) cf = coef[3];
-      cf = __hiloint2double(__double2hiint(cf) ^ (int)((e >> 15) << 31), __double2loint(cf));
-      const double2 x = xs[(e & 0x7fffu) * 8 + l];
-      acc.x = fma(cf, x.x, acc.x);
-      acc.y = fma(cf, x.y, acc.y);
-    }
+__device__ __forceinline__ void hop_entry(uint32_t t, const unsigned char* __restrict__ xs_a,
+                                          const unsigned char* __restrict__ xs_b,
+                                          const double (&coef)[kTileMaxCoef], double2& acc_a,
+                                          double2& acc_b) {
+  const uint32_t off = (t >> 9) & 0x3ff80u;  // row * 128
+  double cf = coef[0];
+  if (NC == 2) {
+    if (t & 0x08000000u) cf = coef[1];
+  } else if (NC > 2) {
+    const uint32_t c = (t >> 27) & 3u;
+    if (c == 1) cf = coef[1];
+    if (c == 2) cf = coef[2];
+    if (NC > 3 && c == 3) cf = coef[3];
   }
-  return acc;
+  cf = __hiloint2double(__double2hiint(cf) ^ (int)(t & 0x80000000u), __double2loint(cf));
+  const double2 xa = *reinterpret_cast<const double2*>(xs_a + off);
+  const double2 xb = *reinterpret_cast<const double2*>(xs_b + off);
+  acc_a.x = fma(cf, xa.x, acc_a.x);
+  acc_a.y = fma(cf, xa.y, acc_a.y);
+  acc_b.x = fma(cf, xb.x, acc_b.x);
+  acc_b.y = fma(cf, xb.y, acc_b.y);
 }
 
-__device__ __forceinline__ int header_degree(uint32_t h) {
-  return (int)((h & 0xff) + ((h >> 8) & 0xff) + ((h >> 16) & 0xff) + (h >> 24));
+// All in-tile neighbours of the row whose record quarter this lane holds (rq); max_deg is
+// warp-uniform, shorter rows run into entries that point at the zero row.
+template <int NC>
+__device__ __forceinline__ void tile_hops(const uint4 rq, int max_deg,
+                                          const unsigned char* __restrict__ xs_a,
+                                          const unsigned char* __restrict__ xs_b,
+                                          const double (&coef)[kTileMaxCoef], double2& acc_a,
+                                          double2& acc_b) {
+#pragma unroll
+  for (int w = 1; w <= kTileMaxDeg / 2; ++w) {
+    if (2 * (w - 1) >= max_deg) break;
+    const uint32_t mine = (w & 3) == 0 ? rq.x : (w & 3) == 1 ? rq.y : (w & 3) == 2 ? rq.z : rq.w;
+    const uint32_t word = __shfl_sync(0xffffffffu, mine, w >> 2, 4);
+    hop_entry<NC>(word << 16, xs_a, xs_b, coef, acc_a, acc_b);
+    hop_entry<NC>(word, xs_a, xs_b, coef, acc_a, acc_b);
+  }
 }
 
 template <int NC>
 __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const SweepArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  double2* xs = reinterpret_cast<double2*>(smem_raw);
+  double2* xs = reinterpret_cast<double2*>(smem_raw);  // (max_tile_rows + 1) x 8 double2
   __shared__ uint64_t bar;
   __shared__ int s_tile;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int l = lane & 7, sg = lane >> 3;
+  const int q = lane & 3, slot = lane >> 2;
+  const int ca = q + 4 * (slot & 1), cb = ca ^ 4;  // the two chunks of this lane
+  const unsigned char* xs_a = smem_raw + ca * 16;
+  const unsigned char* xs_b = smem_raw + cb * 16;
   if (tid == 0) mbar_init(&bar, 1);
   __syncthreads();
   unsigned parity = 0;
   double2* scratch = a.scratch + (size_t)blockIdx.x * a.max_tile_rows * 8;
   const size_t panel_stride = (size_t)a.n * 8;  // double2 per panel
+  constexpr int kRowsPerPass = (kTileThreads / 32) * 8;
 
   for (;;) {
     if (tid == 0) s_tile = atomicAdd(a.counter, 1);
@@ -136,7 +154,10 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
     if (tile >= a.n_tiles) break;
     const int row0 = __ldg(a.tile_row0 + tile);
     const int nrows = __ldg(a.tile_row0 + tile + 1) - row0;
-    const uint2* rec = a.records + (size_t)__ldg(a.tile_rec0 + tile) * 8;
+    const uint4* rec = reinterpret_cast<const uint4*>(a.records) +
+                       (size_t)__ldg(a.tile_rec0 + tile) * 4;
+    if (tid < 8) xs[nrows * 8 + tid] = make_double2(0.0, 0.0);  // the zero row
+    __syncthreads();
 
     for (int panel = 0; panel < a.n_panels; ++panel) {
       const double2* X1 = a.X1 + panel * panel_stride;
@@ -152,35 +173,39 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
       }
 
       // ---- phase 2: b_k = P_k + p_k (O_l + DM) b_{k+1} -----------------------------------------
-      for (int base = warp * 4; base < nrows; base += kGroups) {
-        const int li = base + sg;
-        const bool active = li < nrows;
-        const int row = row0 + li;
-        int dst = row;
-        double2 b = make_double2(0.0, 0.0);
+      for (int base = warp * 8; base < nrows; base += kRowsPerPass) {
+        const int t = base + slot;
+        const bool active = t < nrows;
+        uint4 rq = make_uint4(0u, 0u, 0u, 0u);
+        if (active) rq = __ldg(rec + (size_t)t * 4 + q);
+        const uint32_t header = __shfl_sync(0xffffffffu, rq.x, 0, 4);
+        const int rid = header & 0x7ff;
+        const int row = row0 + rid;
+        double2 ba = make_double2(0.0, 0.0), bb = ba;
         if (a.mode == MODE_INIT) {
           if (active) {
-            const double2 v = __ldcs(V + (size_t)row * 8 + l);
-            b = make_double2(a.cK * v.x, a.cK * v.y);
+            const double2 va = __ldcs(V + (size_t)row * 8 + ca);
+            const double2 vb = __ldcs(V + (size_t)row * 8 + cb);
+            ba = make_double2(a.cK * va.x, a.cK * va.y);
+            bb = make_double2(a.cK * vb.x, a.cK * vb.y);
           }
         } else {
-          uint2 rec2 = make_uint2(0u, 0u);
           int e0 = 0, e1 = 0;
-          double2 pk = make_double2(0.0, 0.0);
+          double2 pka = ba, pkb = ba;
           if (active) {
-            rec2 = __ldg(rec + (size_t)li * 8 + l);
             e0 = __ldg(a.dm_row_ptr + row);
             e1 = __ldg(a.dm_row_ptr + row + 1);
-            pk = __ldcs(Pk + (size_t)row * 8 + l);
+            pka = __ldcs(Pk + (size_t)row * 8 + ca);
+            pkb = __ldcs(Pk + (size_t)row * 8 + cb);
           }
-          const uint32_t header = __shfl_sync(0xffffffffu, rec2.x, 0, 8);
-          const int max_deg = __reduce_max_sync(0xffffffffu, header_degree(header));
+          const int max_deg =
+              __reduce_max_sync(0xffffffffu, active ? (int)((header >> 16) & 0x1f) : 0);
+          double2 acc_a = ba, acc_b = ba;
           // diagonal + cross-cut entries: columns inside the tile come from shared memory
-          double2 acc = make_double2(0.0, 0.0);
           const int ndm = e1 - e0;
           const int max_dm = __reduce_max_sync(0xffffffffu, ndm);
-          for (int off = 0; off < max_dm; off += 8) {
-            const int e = e0 + off + l;
+          for (int off = 0; off < max_dm; off += 4) {
+            const int e = e0 + off + q;
             int cc = 0;
             double vv = 0.0;
             if (e < e1) {
@@ -189,30 +214,42 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
             }
             const int rem = ndm - off;
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
+            for (int j = 0; j < 4; ++j) {
               if (off + j >= max_dm) break;
-              const int cj = __shfl_sync(0xffffffffu, cc, j, 8);
-              const double vj = __shfl_sync(0xffffffffu, vv, j, 8);
+              const int cj = __shfl_sync(0xffffffffu, cc, j, 4);
+              const double vj = __shfl_sync(0xffffffffu, vv, j, 4);
               if (j < rem) {
                 const unsigned u = (unsigned)(cj - row0);
-                const double2 x = (u < (unsigned)nrows) ? xs[u * 8 + l]
-                                                        : __ldg(X1 + (size_t)cj * 8 + l);
-                acc.x = fma(vj, x.x, acc.x);
-                acc.y = fma(vj, x.y, acc.y);
+                double2 xa, xb;
+                if (u < (unsigned)nrows) {
+                  xa = xs[u * 8 + ca];
+                  xb = xs[u * 8 + cb];
+                } else {
+                  xa = __ldg(X1 + (size_t)cj * 8 + ca);
+                  xb = __ldg(X1 + (size_t)cj * 8 + cb);
+                }
+                acc_a.x = fma(vj, xa.x, acc_a.x);
+                acc_a.y = fma(vj, xa.y, acc_a.y);
+                acc_b.x = fma(vj, xb.x, acc_b.x);
+                acc_b.y = fma(vj, xb.y, acc_b.y);
               }
             }
           }
-          const double2 hop = tile_hops<NC>(xs, rec2, header, max_deg, l, a.coef);
-          b.x = fma(a.pf, acc.x + hop.x, pk.x);
-          b.y = fma(a.pf, acc.y + hop.y, pk.y);
+          tile_hops<NC>(rq, max_deg, xs_a, xs_b, a.coef, acc_a, acc_b);
+          ba = make_double2(fma(a.pf, acc_a.x, pka.x), fma(a.pf, acc_a.y, pka.y));
+          bb = make_double2(fma(a.pf, acc_b.x, pkb.x), fma(a.pf, acc_b.y, pkb.y));
         }
         if (active) {
-          if (a.out_perm) dst = __ldg(a.pi + row);
+          const int dst = a.out_perm ? __ldg(a.pi + row) : row;
           if (a.mode == MODE_LAST) {
-            *reinterpret_cast<double2*>(a.W + (size_t)dst * a.w_ld + panel * kTilePanel + 2 * l) = b;
+            double* w = a.W + (size_t)dst * a.w_ld + panel * kTilePanel;
+            *reinterpret_cast<double2*>(w + 2 * ca) = ba;
+            *reinterpret_cast<double2*>(w + 2 * cb) = bb;
           } else {
-            __stcs(Bout + (size_t)dst * 8 + l, b);
-            scratch[li * 8 + l] = b;
+            __stcs(Bout + (size_t)dst * 8 + ca, ba);
+            __stcs(Bout + (size_t)dst * 8 + cb, bb);
+            scratch[rid * 8 + ca] = ba;
+            scratch[rid * 8 + cb] = bb;
           }
         }
       }
@@ -230,32 +267,49 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
       parity ^= 1u;
 
       // ---- phase 3: P_{k-1} = c_{k-1} V + p_{k-1} O_l b_k + q_{k-1} b_k + r b_{k+1} -----------------
-      for (int base = warp * 4; base < nrows; base += kGroups) {
-        const int li = base + sg;
-        const bool active = li < nrows;
-        const int row = row0 + li;
-        uint2 rec2 = make_uint2(0u, 0u);
-        double2 own = make_double2(0.0, 0.0), x1 = own, v = own;
+      for (int base = warp * 8; base < nrows; base += kRowsPerPass) {
+        const int t = base + slot;
+        const bool active = t < nrows;
+        uint4 rq = make_uint4(0u, 0u, 0u, 0u);
+        if (active) rq = __ldg(rec + (size_t)t * 4 + q);
+        const uint32_t header = __shfl_sync(0xffffffffu, rq.x, 0, 4);
+        const int rid = header & 0x7ff;
+        const int row = row0 + rid;
+        const double2 zero = make_double2(0.0, 0.0);
+        double2 x1a = zero, x1b = zero, va = zero, vb = zero;
         int dst = row;
         if (active) {
-          rec2 = __ldg(rec + (size_t)li * 8 + l);
-          if (a.rs != 0.0) x1 = __ldg(X1 + (size_t)row * 8 + l);
-          if (a.cs != 0.0) v = __ldcs(V + (size_t)row * 8 + l);
+          if (a.rs != 0.0) {
+            x1a = __ldg(X1 + (size_t)row * 8 + ca);
+            x1b = __ldg(X1 + (size_t)row * 8 + cb);
+          }
+          if (a.cs != 0.0) {
+            va = __ldcs(V + (size_t)row * 8 + ca);
+            vb = __ldcs(V + (size_t)row * 8 + cb);
+          }
           if (a.out_perm) dst = __ldg(a.pi + row);
-          own = xs[li * 8 + l];
         }
-        const uint32_t header = __shfl_sync(0xffffffffu, rec2.x, 0, 8);
-        const int max_deg = __reduce_max_sync(0xffffffffu, header_degree(header));
-        const double2 hop = tile_hops<NC>(xs, rec2, header, max_deg, l, a.coef);
+        const int max_deg =
+            __reduce_max_sync(0xffffffffu, active ? (int)((header >> 16) & 0x1f) : 0);
+        double2 acc_a = zero, acc_b = zero;
+        tile_hops<NC>(rq, max_deg, xs_a, xs_b, a.coef, acc_a, acc_b);
         if (active) {
-          double2 y;
-          y.x = fma(a.ps, hop.x, a.qs * own.x);
-          y.y = fma(a.ps, hop.y, a.qs * own.y);
-          y.x = fma(a.rs, x1.x, y.x);
-          y.y = fma(a.rs, x1.y, y.y);
-          y.x = fma(a.cs, v.x, y.x);
-          y.y = fma(a.cs, v.y, y.y);
-          __stcs(Pout + (size_t)dst * 8 + l, y);
+          const double2 oa = xs[rid * 8 + ca], ob = xs[rid * 8 + cb];
+          double2 ya, yb;
+          ya.x = fma(a.ps, acc_a.x, a.qs * oa.x);
+          ya.y = fma(a.ps, acc_a.y, a.qs * oa.y);
+          yb.x = fma(a.ps, acc_b.x, a.qs * ob.x);
+          yb.y = fma(a.ps, acc_b.y, a.qs * ob.y);
+          ya.x = fma(a.rs, x1a.x, ya.x);
+          ya.y = fma(a.rs, x1a.y, ya.y);
+          yb.x = fma(a.rs, x1b.x, yb.x);
+          yb.y = fma(a.rs, x1b.y, yb.y);
+          ya.x = fma(a.cs, va.x, ya.x);
+          ya.y = fma(a.cs, va.y, ya.y);
+          yb.x = fma(a.cs, vb.x, yb.x);
+          yb.y = fma(a.cs, vb.y, yb.y);
+          __stcs(Pout + (size_t)dst * 8 + ca, ya);
+          __stcs(Pout + (size_t)dst * 8 + cb, yb);
         }
       }
       __syncthreads();  // all reads of xs done before the next bulk copy
@@ -289,7 +343,7 @@ int launch_sweep(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
 
 int sweep(const TiledPlan* p, int layout, SweepArgs a, cudaStream_t st) {
   const TiledLayout& L = p->lay[layout];
-  a.records = reinterpret_cast<const uint2*>(L.d_records);
+  a.records = L.d_records;
   a.dm_row_ptr = L.d_dm_row_ptr;
   a.dm_col = L.d_dm_col;
   a.dm_val = L.d_dm_val;
@@ -320,7 +374,7 @@ int configure_one(TiledPlan* p, int* occ) {
 }  // namespace
 
 int tiled_configure_launch(TiledPlan* p) {
-  p->smem_bytes = (size_t)p->max_tile_rows * 128;
+  p->smem_bytes = (size_t)(p->max_tile_rows + 1) * 128;  // + the zero row
   int occ = 0, rc;
   if ((rc = configure_one<1>(p, &occ))) return rc;
   if ((rc = configure_one<2>(p, &occ))) return rc;
