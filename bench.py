@@ -244,7 +244,10 @@ def run_cuda(args):
     w = workloads.make_workload(args.config, seed=replica_seed(args.config, rank))
     t0 = time.perf_counter()
     basis = P.polfed_build_basis(w.n_sites, w.n_up)
-    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense)
+    tiled = args.format == "tiled" or (args.format == "auto" and w.n_up >= 0 and w.s in (16, 32)
+                                       and not w.dot_bits)
+    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense,
+                                     fmt=P.FORMAT_TILED if tiled else P.FORMAT_CSR)
     torch.cuda.synchronize()
     build_s = time.perf_counter() - t0
     n, nnz, s, K = ham.n, ham.nnz, w.s, args.order
@@ -257,7 +260,8 @@ def run_cuda(args):
     V = torch.randn(n, s, dtype=torch.float64, device="cuda", generator=gen)
     V /= V.norm(dim=0, keepdim=True)
     W = torch.empty_like(V)
-    work = torch.empty(2 * n * s, dtype=torch.float64, device="cuda")
+    work = torch.empty(P.polfed_filter_workspace_bytes_ham(ham, s) // 8, dtype=torch.float64,
+                       device="cuda")
 
     def one_pass():
         P.polfed_filter_apply(ham, a, b, coeffs, s, V, W, work)
@@ -281,20 +285,37 @@ def run_cuda(args):
         ms = e0.elapsed_time(e1)
         # dominant kernel alone: back-to-back recurrence launches, events on the launching stream
         n_l = max(10, min(200, int(0.5e12 / max(step_bytes(n, nnz, s), 1))))
-        B1, B2 = work[: n * s].view(n, s), work[n * s:].view(n, s)
-        B1.copy_(V)
-        B2.copy_(V)
-        for _ in range(3):
-            P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, -1.0, 1e-3, B1, B2, V, B2)
-            B1, B2 = B2, B1
         k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        k0.record()
-        for _ in range(n_l):
-            P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, -1.0, 1e-3, B1, B2, V, B2)
-            B1, B2 = B2, B1
-        k1.record()
-        torch.cuda.synchronize()
-        kernel_ms = k0.elapsed_time(k1) / n_l
+        if tiled:
+            # one sweep launch per recurrence step; the library has no single-sweep entry point,
+            # so time two filter orders and divide the difference by the extra launches (the
+            # pack kernel and the special first/last sweeps cancel).  All coefficients non-zero
+            # so that every sweep reads V (the full-step byte count).
+            c_short = np.full(9, 1e-3)
+            c_long = np.full(9 + n_l, 1e-3)
+            t_pair = []
+            for cc in (c_short, c_long):
+                P.polfed_filter_apply(ham, a, b, cc, s, V, W, work)
+                k0.record()
+                P.polfed_filter_apply(ham, a, b, cc, s, V, W, work)
+                k1.record()
+                torch.cuda.synchronize()
+                t_pair.append(k0.elapsed_time(k1))
+            kernel_ms = (t_pair[1] - t_pair[0]) / n_l
+        else:
+            B1, B2 = work[: n * s].view(n, s), work[n * s: 2 * n * s].view(n, s)
+            B1.copy_(V)
+            B2.copy_(V)
+            for _ in range(3):
+                P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, -1.0, 1e-3, B1, B2, V, B2)
+                B1, B2 = B2, B1
+            k0.record()
+            for _ in range(n_l):
+                P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, -1.0, 1e-3, B1, B2, V, B2)
+                B1, B2 = B2, B1
+            k1.record()
+            torch.cuda.synchronize()
+            kernel_ms = k0.elapsed_time(k1) / n_l
     ms = reduce_max(ms, "cuda")
     value = whole_job_gbs(pass_bytes(n, nnz, s, coeffs) * args.steps, world, ms * 1e-3)
 
@@ -324,7 +345,7 @@ def run_cuda(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOAD_NAMES[args.config], "N": n, "nnz": nnz, "s": s,
-                       "filter_order_per_step": K, "format": "csr",
+                       "filter_order_per_step": K, "format": "tiled" if tiled else "csr",
                        "bytes_per_fused_launch": step_bytes(n, nnz, s),
                        "l2": "inputs exceed L2 (no flush)" if step_bytes(n, nnz, s) > 4 * 126e6
                              else "working set fits L2; not flushed (the filter re-reads it by design)",
@@ -334,13 +355,15 @@ def run_cuda(args):
             "frac_of_nominal_8TBps": value / world / NOMINAL_HBM_GBS,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * s * n,
                     "d2h_bytes_per_step": 8 * s * n, "steps": e2e_steps, "checksum": checksum},
-            "gpu_launches": args.steps * (K + 1),
+            "gpu_launches": args.steps * (K + 2 if tiled else K + 1),
             "clocks": clocks.summary(),
-            "roofline": {"bound": "hbm", "kernel": "fused_step_kernel", "achieved": achieved,
+            "roofline": {"bound": "hbm",
+                         "kernel": "tiled_sweep_kernel" if tiled else "fused_step_kernel", "achieved": achieved,
                          "peak": peak, "peak_source": peak_src, "unit": UNIT,
                          "frac": achieved / peak, "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS,
                          "launch_ms": kernel_ms, "launches_timed": n_l,
-                         "traffic": recorded_traffic(WORKLOAD_NAMES[args.config])},
+                         "traffic": recorded_traffic(WORKLOAD_NAMES[args.config]
+                                                    + ("/tiled" if tiled else "/csr"))},
         }
         if world == 1 and args.eigs:
             del Vh, Wh, V
@@ -388,6 +411,8 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--order", type=int, default=64, help="filter order K per step")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--format", default="auto", choices=["auto", "csr", "tiled"],
+                    help="auto: the tiled format where the library supports it, else CSR")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--eigs", default="1,2,3",
                     help="configs whose full eigen-solve is timed at N=1 ('' to skip; 4 takes minutes)")
