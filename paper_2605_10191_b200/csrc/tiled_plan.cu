@@ -1,5 +1,6 @@
 // Construction of the tiled format (tiled.cuh): term classification, per-class neighbour
-// records, tile table, the layout permutation and the two diagonal + cross-cut CSR parts.
+// records in processing order, tile table, the position maps between the two layouts and the
+// caller's row order, and the diagonal + cross-cut part of each layout.
 #include <algorithm>
 #include <new>
 
@@ -12,7 +13,7 @@ int tiled_configure_launch(TiledPlan* plan);  // tiled_sweep.cu
 
 namespace {
 
-// Row of state x in the layout with the site order reversed.
+// Row of state x in the ascending order of the states with the site order reversed.
 __global__ void __launch_bounds__(256) reverse_rank_kernel(int64_t n, int n_sites, int n_up,
                                                            const uint64_t* __restrict__ states,
                                                            int32_t* __restrict__ pi) {
@@ -20,6 +21,73 @@ __global__ void __launch_bounds__(256) reverse_rank_kernel(int64_t n, int n_site
   if (r >= n) return;
   const uint64_t y = __brevll(states[r]) >> (64 - n_sites);
   pi[r] = (int32_t)rank_state(y, n_sites, n_up);
+}
+
+// Ascending row (of one layout) -> position: one CTA per tile applies the class permutation.
+__global__ void __launch_bounds__(256) position_kernel(const int32_t* __restrict__ tile_row0,
+                                                       const int32_t* __restrict__ tile_rec0,
+                                                       const int32_t* __restrict__ inv_sigma,
+                                                       int32_t* __restrict__ pos) {
+  const int row0 = tile_row0[blockIdx.x], nrows = tile_row0[blockIdx.x + 1] - row0;
+  const int rec0 = tile_rec0[blockIdx.x];
+  for (int i = threadIdx.x; i < nrows; i += blockDim.x) pos[row0 + i] = row0 + inv_sigma[rec0 + i];
+}
+
+// pos0/pos1: position of an ascending row of layout 0 / layout 1; pi: layout-0 row -> layout-1 row.
+__global__ void __launch_bounds__(256) maps_kernel(int64_t n, const int32_t* __restrict__ pi,
+                                                   const int32_t* __restrict__ pos0,
+                                                   const int32_t* __restrict__ pos1,
+                                                   int32_t* to_other0, int32_t* to_other1,
+                                                   int32_t* to_nat0, int32_t* to_nat1,
+                                                   int32_t* from_nat0, int32_t* from_nat1) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= n) return;
+  const int32_t p0 = pos0[r], p1 = pos1[pi[r]];
+  to_other0[p0] = p1;
+  to_other1[p1] = p0;
+  to_nat0[p0] = (int32_t)r;
+  to_nat1[p1] = (int32_t)r;
+  from_nat0[r] = p0;
+  from_nat1[r] = p1;
+}
+
+__global__ void __launch_bounds__(256) max_offdiag_kernel(int64_t n, const int32_t* __restrict__ row_ptr,
+                                                          int* out) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int v = (r < n) ? row_ptr[r + 1] - row_ptr[r] - 1 : 0;
+  v = __reduce_max_sync(0xffffffffu, v);
+  if ((threadIdx.x & 31) == 0) atomicMax(out, v);
+}
+
+// CSR (ascending rows of this layout, diagonal always stored) -> diagonal + ELL by position.
+__global__ void __launch_bounds__(256) dm_ell_kernel(int64_t n, int n_cross,
+                                                     const int32_t* __restrict__ row_ptr,
+                                                     const int32_t* __restrict__ col,
+                                                     const double* __restrict__ val,
+                                                     const int32_t* __restrict__ pos,
+                                                     double* __restrict__ diag,
+                                                     int32_t* __restrict__ cc_col,
+                                                     double* __restrict__ cc_val) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= n) return;
+  const int32_t p = pos[r];
+  int slot = 0;
+  double d = 0.0;
+  for (int e = row_ptr[r]; e < row_ptr[r + 1]; ++e) {
+    const int32_t c = col[e];
+    if (c == (int32_t)r) {
+      d += val[e];
+    } else {
+      cc_col[(size_t)slot * n + p] = pos[c];
+      cc_val[(size_t)slot * n + p] = val[e];
+      ++slot;
+    }
+  }
+  diag[p] = d;
+  for (; slot < n_cross; ++slot) {
+    cc_col[(size_t)slot * n + p] = -1;
+    cc_val[(size_t)slot * n + p] = 0.0;
+  }
 }
 
 inline bool off_diagonal(int kind) { return kind >= POLFED_TERM_EXCH; }
@@ -45,15 +113,19 @@ int upload(T** d, const std::vector<T>& h) {
   return POLFED_OK;
 }
 
+struct Entry {
+  uint32_t nbr;   // class rank of the neighbour (ascending order inside the class)
+  uint32_t cls;   // amplitude class
+  uint32_t sign;  // 1 = negative
+};
+
 // Records of one layout: `low` holds the tile-local hops with sites already in this layout's
 // numbering (all < m).  Class k (k particles on the low m sites) owns records
-// class_off[k] .. class_off[k+1]; they are sorted by falling degree so that the rows a warp
-// works on together have (nearly) the same number of neighbours.  Record = 16 words:
-//   word 0      row index inside the tile (bits 0-10) | degree (bits 16-20)
-//   words 1-12  24 entries of 16 bits: neighbour row (bits 0-10) | amplitude class (bits 11-12)
-//               | sign (bit 15); unused entries point at the zero row (index = rows of the class)
+// class_off[k] .. class_off[k+1].  Inside a class the rows are put in processing order (falling
+// degree); inv_sigma[class_off[k] + ascending rank] = position inside the class.
 int build_records(int m, const std::vector<DevTerm>& low, TiledLayout* lay,
-                  std::vector<uint32_t>* rec, const std::vector<int>& class_off) {
+                  std::vector<uint32_t>* rec, std::vector<int32_t>* inv_sigma,
+                  const std::vector<int>& class_off) {
   lay->n_coef = 0;
   std::vector<int> cls(low.size(), -1);
   for (size_t t = 0; t < low.size(); ++t) {
@@ -70,11 +142,13 @@ int build_records(int m, const std::vector<DevTerm>& low, TiledLayout* lay,
     }
     cls[t] = c;
   }
-  rec->assign((size_t)(1u << m) * kTileRecWords, 0u);
-  std::vector<std::vector<uint16_t>> ent((size_t)1 << m);  // by class_off[k] + class_rank(l)
-  for (uint32_t l = 0; l < (1u << m); ++l) {
+  const size_t n_cfg = (size_t)1 << m;
+  rec->assign(n_cfg * kTileRecWords, 0u);
+  inv_sigma->assign(n_cfg, 0);
+  std::vector<std::vector<Entry>> ent(n_cfg);  // by class_off[k] + class_rank(l)
+  for (uint32_t l = 0; l < n_cfg; ++l) {
     const int k = __builtin_popcount(l);
-    std::vector<uint16_t>& e = ent[(size_t)class_off[k] + class_rank(l)];
+    std::vector<Entry>& e = ent[(size_t)class_off[k] + class_rank(l)];
     for (size_t t = 0; t < low.size(); ++t) {
       if (cls[t] < 0) continue;
       const int i = low[t].i, j = low[t].j;
@@ -86,7 +160,7 @@ int build_records(int m, const std::vector<DevTerm>& low, TiledLayout* lay,
         const uint32_t between = ((1u << hi) - 1u) & ~((2u << lo) - 1u);
         sign ^= (uint32_t)__builtin_popcount(l & between) & 1u;
       }
-      e.push_back((uint16_t)(class_rank(l2) | ((uint32_t)cls[t] << 11) | (sign << 15)));
+      e.push_back(Entry{class_rank(l2), (uint32_t)cls[t], sign});
     }
     if ((int)e.size() > kTileMaxDeg)
       return fail(POLFED_EINVAL, "tiled format: more than %d hops inside a tile for one state",
@@ -99,32 +173,56 @@ int build_records(int m, const std::vector<DevTerm>& low, TiledLayout* lay,
     std::stable_sort(order.begin(), order.end(), [&](int x, int y) {
       return ent[(size_t)class_off[k] + x].size() > ent[(size_t)class_off[k] + y].size();
     });
+    int32_t* inv = inv_sigma->data() + class_off[k];
+    for (int t = 0; t < n_k; ++t) inv[order[t]] = t;
     for (int t = 0; t < n_k; ++t) {
-      const std::vector<uint16_t>& e = ent[(size_t)class_off[k] + order[t]];
+      const std::vector<Entry>& e = ent[(size_t)class_off[k] + order[t]];
       uint32_t* w = rec->data() + ((size_t)class_off[k] + t) * kTileRecWords;
-      w[0] = (uint32_t)order[t] | ((uint32_t)e.size() << 16);
+      w[0] = (uint32_t)e.size();
       for (int j = 0; j < kTileMaxDeg; ++j) {
-        const uint32_t v = j < (int)e.size() ? e[j] : (uint32_t)n_k;  // zero row
-        w[1 + (j >> 1)] |= v << (16 * (j & 1));
+        const bool used = j < (int)e.size();
+        const uint32_t pos = used ? (uint32_t)inv[e[j].nbr] : (uint32_t)n_k;  // zero row
+        const uint32_t c = used ? e[j].cls : 0u, sg = used ? e[j].sign : 0u;
+        uint32_t& word = w[1 + (j >> 1)];
+        if ((j & 1) == 0) word |= (pos << 7) | c | (sg << 30);
+        else word |= (pos << 18) | (c << 2) | (sg << 31);
       }
     }
   }
   return POLFED_OK;
 }
 
+void free_layout(TiledLayout& l) {
+  cudaFree(l.d_records);
+  cudaFree(l.d_diag);
+  cudaFree(l.d_cc_col);
+  cudaFree(l.d_cc_val);
+  cudaFree(l.d_to_other);
+  cudaFree(l.d_to_natural);
+  cudaFree(l.d_from_natural);
+  l = TiledLayout{};
+}
+
+struct DeviceTemp {  // frees what it holds at scope exit
+  std::vector<void*> p;
+  ~DeviceTemp() {
+    for (void* q : p) cudaFree(q);
+  }
+  template <class T>
+  cudaError_t alloc(T** out, size_t count) {
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(out), sizeof(T) * (count ? count : 1));
+    if (e == cudaSuccess) p.push_back(*out);
+    return e;
+  }
+};
+
 }  // namespace
 
 void destroy_tiled_plan(TiledPlan* p) {
   if (!p) return;
-  for (auto& l : p->lay) {
-    cudaFree(l.d_dm_row_ptr);
-    cudaFree(l.d_dm_col);
-    cudaFree(l.d_dm_val);
-    cudaFree(l.d_records);
-  }
+  for (auto& l : p->lay) free_layout(l);
   cudaFree(p->d_tile_row0);
   cudaFree(p->d_tile_rec0);
-  cudaFree(p->d_pi);
   cudaFree(p->d_counter);
   delete p;
 }
@@ -141,7 +239,7 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
   int rc = ensure_binomials();
   if (rc) return rc;
 
-  // classify: A = inside layout 0's low sites, B = inside layout 1's, else cross-cut
+  // classify: inside layout 0's low sites, inside layout 1's, else diagonal / cross-cut
   std::vector<DevTerm> low[2], dm[2];
   for (const DevTerm& t : terms) {
     DevTerm r = t;  // the same term with the site order reversed
@@ -174,6 +272,8 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
   p->n_up = n_up;
   p->m = m;
   p->n = basis->dim;
+  const int64_t n = p->n;
+  const size_t n_alloc = (size_t)(n ? n : 1);
 
   std::vector<int> class_off(m + 2, 0);
   for (int k = 0; k <= m; ++k) class_off[k + 1] = class_off[k] + (int)host_binom(m, k);
@@ -189,29 +289,85 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
     p->max_tile_rows = std::max(p->max_tile_rows, nr);
   }
   row0.push_back((int32_t)rows);
-  if (rows != p->n) return fail(POLFED_ECUDA, "tiled format: tile table does not cover the basis");
+  if (rows != n) return fail(POLFED_ECUDA, "tiled format: tile table does not cover the basis");
   p->n_tiles = (int)rec0.size();
   rc = upload(&p->d_tile_row0, row0);
   if (rc) return rc;
   rc = upload(&p->d_tile_rec0, rec0);
   if (rc) return rc;
 
+  DeviceTemp tmp;
+  int32_t* d_pi = nullptr;
+  int32_t* d_pos[2] = {nullptr, nullptr};
+  int* d_max = nullptr;
+  POLFED_CUDA(tmp.alloc(&d_pi, n_alloc));
+  POLFED_CUDA(tmp.alloc(&d_pos[0], n_alloc));
+  POLFED_CUDA(tmp.alloc(&d_pos[1], n_alloc));
+  POLFED_CUDA(tmp.alloc(&d_max, 1));
+  const unsigned row_grid = (unsigned)((n + 255) / 256);
+
   for (int l = 0; l < 2; ++l) {
+    TiledLayout& lay = p->lay[l];
     std::vector<uint32_t> rec;
-    rc = build_records(m, low[l], &p->lay[l], &rec, class_off);
+    std::vector<int32_t> inv_sigma;
+    rc = build_records(m, low[l], &lay, &rec, &inv_sigma, class_off);
     if (rc) return rc;
-    rc = upload(&p->lay[l].d_records, rec);
+    rc = upload(&lay.d_records, rec);
     if (rc) return rc;
-    rc = assemble_csr(basis, dm[l], 0, nullptr, st, &p->lay[l].d_dm_row_ptr, &p->lay[l].d_dm_col,
-                      &p->lay[l].d_dm_val, &p->lay[l].dm_nnz);
+    int32_t* d_inv = nullptr;
+    POLFED_CUDA(tmp.alloc(&d_inv, inv_sigma.size()));
+    POLFED_CUDA(cudaMemcpyAsync(d_inv, inv_sigma.data(), sizeof(int32_t) * inv_sigma.size(),
+                                cudaMemcpyHostToDevice, st));
+    if (p->n_tiles > 0) {
+      position_kernel<<<(unsigned)p->n_tiles, 256, 0, st>>>(p->d_tile_row0, p->d_tile_rec0, d_inv,
+                                                            d_pos[l]);
+      POLFED_LAUNCH_CHECK("position_kernel");
+    }
+    POLFED_CUDA(cudaStreamSynchronize(st));  // inv_sigma (host) is read by the copy above
+
+    // diagonal + cross-cut part: CSR over the ascending rows of this layout, then by position
+    int32_t* d_rp = nullptr;
+    int32_t* d_col = nullptr;
+    double* d_val = nullptr;
+    long long nnz = 0;
+    rc = assemble_csr(basis, dm[l], 0, nullptr, st, &d_rp, &d_col, &d_val, &nnz);
     if (rc) return rc;
+    tmp.p.push_back(d_rp);
+    tmp.p.push_back(d_col);
+    tmp.p.push_back(d_val);
+    int n_cross = 0;
+    if (n > 0) {
+      POLFED_CUDA(cudaMemsetAsync(d_max, 0, sizeof(int), st));
+      max_offdiag_kernel<<<row_grid, 256, 0, st>>>(n, d_rp, d_max);
+      POLFED_LAUNCH_CHECK("max_offdiag_kernel");
+      POLFED_CUDA(cudaMemcpyAsync(&n_cross, d_max, sizeof(int), cudaMemcpyDeviceToHost, st));
+      POLFED_CUDA(cudaStreamSynchronize(st));
+    }
+    if (n_cross > kTileMaxCross)
+      return fail(POLFED_EINVAL, "tiled format: %d hops of one state cross the cut (limit %d)",
+                  n_cross, kTileMaxCross);
+    lay.n_cross = n_cross;
+    POLFED_CUDA(cudaMalloc(&lay.d_diag, sizeof(double) * n_alloc));
+    POLFED_CUDA(cudaMalloc(&lay.d_cc_col, sizeof(int32_t) * n_alloc * (size_t)std::max(n_cross, 1)));
+    POLFED_CUDA(cudaMalloc(&lay.d_cc_val, sizeof(double) * n_alloc * (size_t)std::max(n_cross, 1)));
+    POLFED_CUDA(cudaMalloc(&lay.d_to_other, sizeof(int32_t) * n_alloc));
+    POLFED_CUDA(cudaMalloc(&lay.d_to_natural, sizeof(int32_t) * n_alloc));
+    POLFED_CUDA(cudaMalloc(&lay.d_from_natural, sizeof(int32_t) * n_alloc));
+    if (n > 0) {
+      dm_ell_kernel<<<row_grid, 256, 0, st>>>(n, n_cross, d_rp, d_col, d_val, d_pos[l], lay.d_diag,
+                                              lay.d_cc_col, lay.d_cc_val);
+      POLFED_LAUNCH_CHECK("dm_ell_kernel");
+    }
   }
 
-  POLFED_CUDA(cudaMalloc(&p->d_pi, sizeof(int32_t) * (size_t)(p->n ? p->n : 1)));
-  if (p->n > 0) {
-    reverse_rank_kernel<<<(unsigned)((p->n + 255) / 256), 256, 0, st>>>(p->n, L, n_up,
-                                                                       basis->d_states, p->d_pi);
+  if (n > 0) {
+    reverse_rank_kernel<<<row_grid, 256, 0, st>>>(n, L, n_up, basis->d_states, d_pi);
     POLFED_LAUNCH_CHECK("reverse_rank_kernel");
+    maps_kernel<<<row_grid, 256, 0, st>>>(n, d_pi, d_pos[0], d_pos[1], p->lay[0].d_to_other,
+                                          p->lay[1].d_to_other, p->lay[0].d_to_natural,
+                                          p->lay[1].d_to_natural, p->lay[0].d_from_natural,
+                                          p->lay[1].d_from_natural);
+    POLFED_LAUNCH_CHECK("maps_kernel");
   }
   POLFED_CUDA(cudaMalloc(&p->d_counter, sizeof(int)));
   POLFED_CUDA(cudaMemsetAsync(p->d_counter, 0, sizeof(int), st));
