@@ -33,7 +33,10 @@ constexpr int kTileMaxSites = 13;     // C(13,6) rows x 128 B = 219 648 B of sha
 constexpr int kTileRecWords = 16;     // 64-byte record per class row
 constexpr int kTileMaxDeg = 24;       // in-tile neighbours per row (12 entry words)
 constexpr int kTileMaxCoef = 4;       // distinct |amplitude| values per layout
-constexpr int kTileMaxCross = 4;      // cross-cut neighbours per row (ELL width)
+constexpr int kTileMaxCross = 7;      // cross-cut neighbours per row
+constexpr int kTileMaxCrossCoef = 15; // distinct |amplitude| values among the cross-cut hops
+constexpr uint32_t kCrossNone = 0xffffffffu;
+constexpr int kCrossPosBits = 26;     // cross word: bits 0-25 position, 26-29 amplitude, 31 sign
 constexpr int kTilePanel = 16;        // columns per panel: 128-byte rows, conflict-free in smem
 constexpr int kTileThreads = 512;
 
@@ -48,9 +51,12 @@ constexpr int kTileThreads = 512;
 struct TiledLayout {
   uint32_t* d_records = nullptr;      // [2^m][kTileRecWords], class blocks in position order
   double* d_diag = nullptr;           // [n] diagonal of H by position
-  int32_t* d_cc_col = nullptr;        // [n_cross][n] position of the cross-cut neighbour, -1 = none
-  double* d_cc_val = nullptr;         // [n_cross][n]
+  uint32_t* d_side = nullptr;         // [n][side_words]: position in the other layout, then the
+                                      // packed cross-cut neighbours (kCrossNone = none)
+  int side_words = 4;                 // 4 (n_cross <= 3) or 8
   int n_cross = 0;
+  double ccoef[kTileMaxCrossCoef + 1] = {};  // |amplitude| table of the cross-cut hops
+  int n_ccoef = 0;
   int32_t* d_to_other = nullptr;      // [n] position in the other layout
   int32_t* d_to_natural = nullptr;    // [n] row in the caller's order
   int32_t* d_from_natural = nullptr;  // [n] position of the caller's row

@@ -2,6 +2,7 @@
 // records in processing order, tile table, the position maps between the two layouts and the
 // caller's row order, and the diagonal + cross-cut part of each layout.
 #include <algorithm>
+#include <cstring>
 #include <new>
 
 #include "combinadic.cuh"
@@ -39,12 +40,16 @@ __global__ void __launch_bounds__(256) maps_kernel(int64_t n, const int32_t* __r
                                                    const int32_t* __restrict__ pos1,
                                                    int32_t* to_other0, int32_t* to_other1,
                                                    int32_t* to_nat0, int32_t* to_nat1,
-                                                   int32_t* from_nat0, int32_t* from_nat1) {
+                                                   int32_t* from_nat0, int32_t* from_nat1,
+                                                   uint32_t* side0, int sw0, uint32_t* side1,
+                                                   int sw1) {
   const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= n) return;
   const int32_t p0 = pos0[r], p1 = pos1[pi[r]];
   to_other0[p0] = p1;
   to_other1[p1] = p0;
+  side0[(size_t)p0 * sw0] = (uint32_t)p1;
+  side1[(size_t)p1 * sw1] = (uint32_t)p0;
   to_nat0[p0] = (int32_t)r;
   to_nat1[p1] = (int32_t)r;
   from_nat0[r] = p0;
@@ -59,15 +64,38 @@ __global__ void __launch_bounds__(256) max_offdiag_kernel(int64_t n, const int32
   if ((threadIdx.x & 31) == 0) atomicMax(out, v);
 }
 
-// CSR (ascending rows of this layout, diagonal always stored) -> diagonal + ELL by position.
+// Distinct |value| of the off-diagonal CSR entries -> table[0..kTileMaxCrossCoef) (bit patterns,
+// 0 = free slot; insertion order is arbitrary, the packed words below refer to the final slots).
+__global__ void __launch_bounds__(256) cross_coef_kernel(int64_t n, const int32_t* __restrict__ row_ptr,
+                                                         const int32_t* __restrict__ col,
+                                                         const double* __restrict__ val,
+                                                         unsigned long long* table, int* overflow) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= n) return;
+  for (int e = row_ptr[r]; e < row_ptr[r + 1]; ++e) {
+    if (col[e] == (int32_t)r || val[e] == 0.0) continue;
+    const unsigned long long mag = (unsigned long long)__double_as_longlong(fabs(val[e]));
+    int c = 0;
+    for (; c < kTileMaxCrossCoef; ++c) {
+      unsigned long long cur = table[c];
+      if (cur == 0ull) cur = atomicCAS(table + c, 0ull, mag);
+      if (cur == 0ull || cur == mag) break;
+    }
+    if (c == kTileMaxCrossCoef) *overflow = 1;
+  }
+}
+
+// CSR (ascending rows of this layout, diagonal always stored) -> diagonal + packed cross-cut
+// words by position (word 0 of a side record, the position in the other layout, is filled by
+// maps_kernel).
 __global__ void __launch_bounds__(256) dm_ell_kernel(int64_t n, int n_cross,
                                                      const int32_t* __restrict__ row_ptr,
                                                      const int32_t* __restrict__ col,
                                                      const double* __restrict__ val,
                                                      const int32_t* __restrict__ pos,
-                                                     double* __restrict__ diag,
-                                                     int32_t* __restrict__ cc_col,
-                                                     double* __restrict__ cc_val) {
+                                                     const unsigned long long* __restrict__ table,
+                                                     double* __restrict__ diag, int side_words,
+                                                     uint32_t* __restrict__ side) {
   const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= n) return;
   const int32_t p = pos[r];
@@ -77,17 +105,17 @@ __global__ void __launch_bounds__(256) dm_ell_kernel(int64_t n, int n_cross,
     const int32_t c = col[e];
     if (c == (int32_t)r) {
       d += val[e];
-    } else {
-      cc_col[(size_t)slot * n + p] = pos[c];
-      cc_val[(size_t)slot * n + p] = val[e];
+    } else if (val[e] != 0.0) {
+      const unsigned long long mag = (unsigned long long)__double_as_longlong(fabs(val[e]));
+      uint32_t cls = 0;
+      while (cls < (uint32_t)kTileMaxCrossCoef - 1 && table[cls] != mag) ++cls;
+      side[(size_t)p * side_words + 1 + slot] = (uint32_t)pos[c] | (cls << kCrossPosBits) |
+                                                (val[e] < 0.0 ? 0x80000000u : 0u);
       ++slot;
     }
   }
   diag[p] = d;
-  for (; slot < n_cross; ++slot) {
-    cc_col[(size_t)slot * n + p] = -1;
-    cc_val[(size_t)slot * n + p] = 0.0;
-  }
+  for (; slot + 1 < side_words; ++slot) side[(size_t)p * side_words + 1 + slot] = kCrossNone;
 }
 
 inline bool off_diagonal(int kind) { return kind >= POLFED_TERM_EXCH; }
@@ -195,8 +223,7 @@ int build_records(int m, const std::vector<DevTerm>& low, TiledLayout* lay,
 void free_layout(TiledLayout& l) {
   cudaFree(l.d_records);
   cudaFree(l.d_diag);
-  cudaFree(l.d_cc_col);
-  cudaFree(l.d_cc_val);
+  cudaFree(l.d_side);
   cudaFree(l.d_to_other);
   cudaFree(l.d_to_natural);
   cudaFree(l.d_from_natural);
@@ -233,9 +260,9 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
   const int L = basis->n_sites, n_up = basis->n_up;
   if (n_up < 0 || !basis->d_states)
     return fail(POLFED_EINVAL, "tiled format: needs a fixed-particle-number basis");
-  const int m = (L + 1) / 2;
-  if (L < 4 || m > kTileMaxSites)
+  if (L < 4 || L > 2 * kTileMaxSites)
     return fail(POLFED_EINVAL, "tiled format: n_sites=%d not in [4,%d]", L, 2 * kTileMaxSites);
+  const int m = (L + 1) / 2;
   int rc = ensure_binomials();
   if (rc) return rc;
 
@@ -304,6 +331,11 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
   POLFED_CUDA(tmp.alloc(&d_pos[0], n_alloc));
   POLFED_CUDA(tmp.alloc(&d_pos[1], n_alloc));
   POLFED_CUDA(tmp.alloc(&d_max, 1));
+  unsigned long long* d_table = nullptr;
+  POLFED_CUDA(tmp.alloc(&d_table, kTileMaxCrossCoef));
+  if (n >= ((int64_t)1 << kCrossPosBits))
+    return fail(POLFED_EINVAL, "tiled format: dimension %lld needs more than %d position bits",
+                (long long)n, kCrossPosBits);
   const unsigned row_grid = (unsigned)((n + 255) / 256);
 
   for (int l = 0; l < 2; ++l) {
@@ -348,15 +380,35 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
                   n_cross, kTileMaxCross);
     lay.n_cross = n_cross;
     POLFED_CUDA(cudaMalloc(&lay.d_diag, sizeof(double) * n_alloc));
-    POLFED_CUDA(cudaMalloc(&lay.d_cc_col, sizeof(int32_t) * n_alloc * (size_t)std::max(n_cross, 1)));
-    POLFED_CUDA(cudaMalloc(&lay.d_cc_val, sizeof(double) * n_alloc * (size_t)std::max(n_cross, 1)));
+    lay.side_words = n_cross <= 3 ? 4 : 8;
+    POLFED_CUDA(cudaMalloc(&lay.d_side, sizeof(uint32_t) * n_alloc * (size_t)lay.side_words));
     POLFED_CUDA(cudaMalloc(&lay.d_to_other, sizeof(int32_t) * n_alloc));
     POLFED_CUDA(cudaMalloc(&lay.d_to_natural, sizeof(int32_t) * n_alloc));
     POLFED_CUDA(cudaMalloc(&lay.d_from_natural, sizeof(int32_t) * n_alloc));
     if (n > 0) {
-      dm_ell_kernel<<<row_grid, 256, 0, st>>>(n, n_cross, d_rp, d_col, d_val, d_pos[l], lay.d_diag,
-                                              lay.d_cc_col, lay.d_cc_val);
+      POLFED_CUDA(cudaMemsetAsync(d_table, 0, sizeof(unsigned long long) * kTileMaxCrossCoef, st));
+      POLFED_CUDA(cudaMemsetAsync(d_max, 0, sizeof(int), st));
+      cross_coef_kernel<<<row_grid, 256, 0, st>>>(n, d_rp, d_col, d_val, d_table, d_max);
+      POLFED_LAUNCH_CHECK("cross_coef_kernel");
+      dm_ell_kernel<<<row_grid, 256, 0, st>>>(n, n_cross, d_rp, d_col, d_val, d_pos[l], d_table,
+                                              lay.d_diag, lay.side_words, lay.d_side);
       POLFED_LAUNCH_CHECK("dm_ell_kernel");
+      int overflow = 0;
+      unsigned long long table[kTileMaxCrossCoef];
+      POLFED_CUDA(cudaMemcpyAsync(&overflow, d_max, sizeof(int), cudaMemcpyDeviceToHost, st));
+      POLFED_CUDA(cudaMemcpyAsync(table, d_table, sizeof(table), cudaMemcpyDeviceToHost, st));
+      POLFED_CUDA(cudaStreamSynchronize(st));
+      if (overflow)
+        return fail(POLFED_EINVAL,
+                    "tiled format: more than %d distinct hopping amplitudes across the cut",
+                    kTileMaxCrossCoef);
+      lay.n_ccoef = 0;
+      for (int c = 0; c < kTileMaxCrossCoef; ++c) {
+        double mag;
+        memcpy(&mag, &table[c], sizeof(double));
+        lay.ccoef[c] = mag;
+        if (table[c]) lay.n_ccoef = c + 1;
+      }
     }
   }
 
@@ -366,7 +418,9 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
     maps_kernel<<<row_grid, 256, 0, st>>>(n, d_pi, d_pos[0], d_pos[1], p->lay[0].d_to_other,
                                           p->lay[1].d_to_other, p->lay[0].d_to_natural,
                                           p->lay[1].d_to_natural, p->lay[0].d_from_natural,
-                                          p->lay[1].d_from_natural);
+                                          p->lay[1].d_from_natural, p->lay[0].d_side,
+                                          p->lay[0].side_words, p->lay[1].d_side,
+                                          p->lay[1].side_words);
     POLFED_LAUNCH_CHECK("maps_kernel");
   }
   POLFED_CUDA(cudaMalloc(&p->d_counter, sizeof(int)));

@@ -26,9 +26,9 @@ struct SweepArgs {
   const int32_t* tile_rec0;
   const uint32_t* records;  // kTileRecWords words per class row, position order
   const double* diag;       // [n]
-  const int32_t* cc_col;    // [n_cross][n]
-  const double* cc_val;     // [n_cross][n]
-  int n_cross;
+  const uint32_t* side;     // [n][side_words]: other-layout position, packed cross-cut words
+  int side_words;
+  double ccoef[kTileMaxCrossCoef + 1];
   const int32_t* dst_map;   // position -> output row (other layout, or natural for MODE_LAST)
   double coef[kTileMaxCoef];
   const double* X1;  // b_{k+1}, panel-major, this layout
@@ -57,22 +57,41 @@ __device__ __forceinline__ D4 ldg256(const double* p) {  // read-only data, defa
                : "l"(p));
   return r;
 }
-__device__ __forceinline__ D4 ldg256_stream(const double* p) {  // touched once
+// L2 policies: block passes that are touched once per sweep leave L2 first, the per-CTA scratch
+// and the tile of b_{k+1} (read again by phase 3 and by the neighbours' cross-cut hops) last.
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ D4 ldg256_stream(const double* p, uint64_t pol) {  // touched once
   D4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
+  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f64 {%0,%1,%2,%3}, [%4], %5;"
                : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w)
-               : "l"(p));
+               : "l"(p), "l"(pol));
   return r;
+}
+__device__ __forceinline__ void stg256_hint(double* p, const D4& r, uint64_t pol) {
+  asm volatile("st.global.L1::no_allocate.L2::cache_hint.v4.f64 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p),
+               "d"(r.x), "d"(r.y), "d"(r.z), "d"(r.w), "l"(pol)
+               : "memory");
 }
 __device__ __forceinline__ void stg256(double* p, const D4& r) {
   asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(r.x), "d"(r.y), "d"(r.z),
                "d"(r.w)
                : "memory");
 }
-__device__ __forceinline__ void stg256_stream(double* p, const D4& r) {
-  asm volatile("st.global.L1::no_allocate.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(r.x),
-               "d"(r.y), "d"(r.z), "d"(r.w)
-               : "memory");
+__device__ __forceinline__ D4 ldg256_plain_stream(const double* p) {
+  D4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
+               : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w)
+               : "l"(p));
+  return r;
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -87,11 +106,12 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
                "r"(bytes)
                : "memory");
 }
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar) {
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar,
+                                         uint64_t pol) {
   asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-          smem_u32(dst)),
-      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], "
+      "%2, [%3], %4;" ::"r"(smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
       : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
@@ -112,11 +132,12 @@ __device__ __forceinline__ void fence_proxy_async() {
 }
 
 // One thread: bulk-copy `bytes` (a multiple of 128) from global to shared in <= 32 KB pieces.
-__device__ __forceinline__ void tile_load(void* dst, const void* src, unsigned bytes, uint64_t* bar) {
+__device__ __forceinline__ void tile_load(void* dst, const void* src, unsigned bytes, uint64_t* bar,
+                                          uint64_t pol) {
   mbar_expect_tx(bar, bytes);
   for (unsigned at = 0; at < bytes; at += 32768u) {
     const unsigned len = min(32768u, bytes - at);
-    bulk_g2s(static_cast<char*>(dst) + at, static_cast<const char*>(src) + at, len, bar);
+    bulk_g2s(static_cast<char*>(dst) + at, static_cast<const char*>(src) + at, len, bar, pol);
   }
 }
 
@@ -133,11 +154,18 @@ __device__ __forceinline__ double pick_coef(uint32_t cls, const double (&coef)[k
   return cf;
 }
 
-__device__ __forceinline__ void hop_fma(double cf, uint32_t sign_bit31, uint32_t off,
+__device__ __forceinline__ double signed_coef(double cf, uint32_t sign_bit31) {
+  return __hiloint2double(__double2hiint(cf) ^ (int)(sign_bit31 & 0x80000000u), __double2loint(cf));
+}
+
+// One neighbour: position (x 128 bytes) `off`, amplitude class `cls`, sign in bit 31 of `sg`.
+template <int NC>
+__device__ __forceinline__ void hop_fma(uint32_t cls, uint32_t sg, uint32_t off,
                                         const unsigned char* __restrict__ x_first,
-                                        const unsigned char* __restrict__ x_second, double2& acc_f,
+                                        const unsigned char* __restrict__ x_second,
+                                        const double (&coef)[kTileMaxCoef], double2& acc_f,
                                         double2& acc_s) {
-  cf = __hiloint2double(__double2hiint(cf) ^ (int)(sign_bit31 & 0x80000000u), __double2loint(cf));
+  const double cf = signed_coef(pick_coef<NC>(cls, coef), sg);
   const double2 xa = *reinterpret_cast<const double2*>(x_first + off);
   const double2 xb = *reinterpret_cast<const double2*>(x_second + off);
   acc_f.x = fma(cf, xa.x, acc_f.x);
@@ -159,10 +187,10 @@ __device__ __forceinline__ void tile_hops(const uint4 rq, int max_deg,
     if (2 * (w - 1) >= max_deg) break;
     const uint32_t mine = (w & 3) == 0 ? rq.x : (w & 3) == 1 ? rq.y : (w & 3) == 2 ? rq.z : rq.w;
     const uint32_t word = __shfl_sync(0xffffffffu, mine, w >> 2, 4);
-    hop_fma(pick_coef<NC>(word & 3u, coef), word << 1, word & 0x3ff80u, x_first, x_second, acc_f,
-            acc_s);
-    hop_fma(pick_coef<NC>((word >> 2) & 3u, coef), word, (word >> 11) & 0x3ff80u, x_first,
-            x_second, acc_f, acc_s);
+    hop_fma<NC>(word & 3u, word << 1, word & 0x3ff80u, x_first, x_second, coef, acc_f, acc_s);
+    if (2 * w - 1 < max_deg)  // an odd warp-wide degree ends on a half-used word
+      hop_fma<NC>((word >> 2) & 3u, word, (word >> 11) & 0x3ff80u, x_first, x_second, coef, acc_f,
+                  acc_s);
   }
 }
 
@@ -176,7 +204,42 @@ __device__ __forceinline__ D4 to_lohi(const double2 f, const double2 s, bool odd
   return r;
 }
 
-template <int NC>
+__device__ __forceinline__ void d4_zero(D4& r) { r.x = r.y = r.z = r.w = 0.0; }
+__device__ __forceinline__ void d4_fma(double c, const D4& g, D4& acc) {
+  acc.x = fma(c, g.x, acc.x);
+  acc.y = fma(c, g.y, acc.y);
+  acc.z = fma(c, g.z, acc.z);
+  acc.w = fma(c, g.w, acc.w);
+}
+
+constexpr uint32_t kCrossPosMask = (1u << kCrossPosBits) - 1u;
+constexpr int kIterRows = kWarps * kRowsPerIter;  // rows per CTA iteration
+
+// What phase 2 needs of a row before its tile hops: the record quarter, the side record
+// (position in the other layout + first three cross-cut words) and the diagonal.  Loaded one
+// iteration ahead, so that the cross-cut gathers can be issued before the hops.
+struct RowHead {
+  uint4 rq;
+  uint4 side;
+  double dg;
+};
+
+__device__ __forceinline__ RowHead load_head(const uint4* rec, const uint32_t* side_row0,
+                                             int side_words, const double* diag_row0, int pos,
+                                             int nrows, int q) {
+  RowHead h;
+  h.rq = make_uint4(0u, 0u, 0u, 0u);
+  h.side = make_uint4(0u, kCrossNone, kCrossNone, kCrossNone);
+  h.dg = 0.0;
+  if (pos < nrows) {
+    h.rq = __ldg(rec + (size_t)pos * 4 + q);
+    h.side = __ldg(reinterpret_cast<const uint4*>(side_row0 + (size_t)pos * side_words));
+    h.dg = __ldg(diag_row0 + pos);
+  }
+  return h;
+}
+
+template <int NC, int MODE>
 __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const SweepArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];  // (max_tile_rows + 1) x 128 B
   __shared__ uint64_t bar;
@@ -192,6 +255,8 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
   double* scratch = a.scratch + (size_t)blockIdx.x * a.max_tile_rows * kTilePanel;
   const size_t panel_stride = (size_t)a.n * kTilePanel;  // doubles per panel
   const double2 zero2 = make_double2(0.0, 0.0);
+  const int first_pos = warp * kRowsPerIter + slot;
+  const uint64_t pol_first = l2_policy_evict_first(), pol_last = l2_policy_evict_last();
 
   for (;;) {
     if (tid == 0) s_tile = atomicAdd(a.counter, 1);
@@ -202,139 +267,138 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
     const int nrows = __ldg(a.tile_row0 + tile + 1) - row0;
     const uint4* rec = reinterpret_cast<const uint4*>(a.records) +
                        (size_t)__ldg(a.tile_rec0 + tile) * 4;
+    const uint32_t* side = a.side + (size_t)row0 * a.side_words;
+    const double* diag = a.diag + row0;
+    const int32_t* dst_map = a.dst_map + row0;
     if (tid < 8) reinterpret_cast<double2*>(smem_raw)[nrows * 8 + tid] = zero2;  // the zero row
-    const int first_pos = warp * kRowsPerIter + slot;
     __syncthreads();
 
     for (int panel = 0; panel < a.n_panels; ++panel) {
       const double* X1 = a.X1 + panel * panel_stride;
-      const double* Pk = a.Pk + panel * panel_stride;
-      const double* V = a.V + panel * panel_stride;
+      const double* Pk = a.Pk + panel * panel_stride + (size_t)row0 * kTilePanel;
+      const double* V = a.V + panel * panel_stride + (size_t)row0 * kTilePanel;
       double* Bout = a.Bout + panel * panel_stride;
       double* Pout = a.Pout + panel * panel_stride;
 
-      uint4 rq_next = make_uint4(0u, 0u, 0u, 0u);
-      if (first_pos < nrows) rq_next = __ldg(rec + (size_t)first_pos * 4 + q);
-      if (a.mode != MODE_INIT) {
-        if (tid == 0) tile_load(smem_raw, X1 + (size_t)row0 * kTilePanel, (unsigned)nrows * 128u, &bar);
+      if (MODE == MODE_INIT) {
+        // ---- b_K = c_K V ------------------------------------------------------------------------
+        for (int pos = first_pos; pos < nrows; pos += kIterRows) {
+          const int dst = __ldg(dst_map + pos);
+          D4 b = ldg256_stream(V + (size_t)pos * kTilePanel + 4 * q, pol_first);
+          b.x *= a.cK;
+          b.y *= a.cK;
+          b.z *= a.cK;
+          b.w *= a.cK;
+          stg256_hint(Bout + (size_t)dst * kTilePanel + 4 * q, b, pol_first);
+          stg256_hint(scratch + (size_t)pos * kTilePanel + 4 * q, b, pol_last);
+        }
+      } else {
+        // ---- phase 2: b_k = P_k + p_k (O_l + DM) b_{k+1} ---------------------------------------
+        if (tid == 0)
+          tile_load(smem_raw, X1 + (size_t)row0 * kTilePanel, (unsigned)nrows * 128u, &bar,
+                    pol_last);
+        RowHead nx = load_head(rec, side, a.side_words, diag, first_pos, nrows, q);
         mbar_wait(&bar, parity);
         parity ^= 1u;
-      }
-
-      // ---- phase 2: b_k = P_k + p_k (O_l + DM) b_{k+1} -----------------------------------------
-      for (int base = warp * kRowsPerIter; base < nrows; base += kWarps * kRowsPerIter) {
-        const int pos = base + slot;
-        const bool active = pos < nrows;
-        const size_t row = (size_t)row0 + pos;
-        const uint4 rq = rq_next;
-        {
-          const int pos_n = pos + kWarps * kRowsPerIter;
-          if (pos_n < nrows) rq_next = __ldg(rec + (size_t)pos_n * 4 + q);
-        }
-        int dst = 0;
-        if (active) dst = __ldg(a.dst_map + row);
-        D4 b;
-        if (a.mode == MODE_INIT) {
-          b.x = b.y = b.z = b.w = 0.0;
+        for (int base = warp * kRowsPerIter; base < nrows; base += kIterRows) {
+          const int pos = base + slot;
+          const bool active = pos < nrows;
+          const RowHead hd = nx;
+          nx = load_head(rec, side, a.side_words, diag, pos + kIterRows, nrows, q);
+          // this row's stream and the cross-cut rows (other tiles, from L2) fly during the hops
+          D4 pk, g0, g1, g2;
+          d4_zero(pk);
+          d4_zero(g0);
+          d4_zero(g1);
+          d4_zero(g2);
+          int dst = (int)hd.side.x;
           if (active) {
-            const D4 v = ldg256_stream(V + row * kTilePanel + 4 * q);
-            b.x = a.cK * v.x;
-            b.y = a.cK * v.y;
-            b.z = a.cK * v.z;
-            b.w = a.cK * v.w;
+            pk = ldg256_stream(Pk + (size_t)pos * kTilePanel + 4 * q, pol_first);
+            if (MODE == MODE_LAST) dst = __ldg(dst_map + pos);
           }
-        } else {
-          D4 pk;
-          pk.x = pk.y = pk.z = pk.w = 0.0;
-          double dg = 0.0;
-          int cc[kTileMaxCross];
-          double cv[kTileMaxCross];
-#pragma unroll
-          for (int j = 0; j < kTileMaxCross; ++j) {
-            cc[j] = -1;
-            cv[j] = 0.0;
-          }
-          if (active) {
-            pk = ldg256_stream(Pk + row * kTilePanel + 4 * q);
-            dg = __ldg(a.diag + row);
-#pragma unroll
-            for (int j = 0; j < kTileMaxCross; ++j)
-              if (j < a.n_cross) {
-                cc[j] = __ldg(a.cc_col + (size_t)j * a.n + row);
-                cv[j] = __ldg(a.cc_val + (size_t)j * a.n + row);
-              }
-          }
-          const int deg = __shfl_sync(0xffffffffu, (int)rq.x, 0, 4);
-          const int max_deg = __reduce_max_sync(0xffffffffu, active ? deg : 0);
+          if (hd.side.y != kCrossNone)
+            g0 = ldg256(X1 + (size_t)(hd.side.y & kCrossPosMask) * kTilePanel + 4 * q);
+          if (hd.side.z != kCrossNone)
+            g1 = ldg256(X1 + (size_t)(hd.side.z & kCrossPosMask) * kTilePanel + 4 * q);
+          if (hd.side.w != kCrossNone)
+            g2 = ldg256(X1 + (size_t)(hd.side.w & kCrossPosMask) * kTilePanel + 4 * q);
+          const int deg = __shfl_sync(0xffffffffu, (int)hd.rq.x, 0, 4);
+          const int max_deg = __reduce_max_sync(0xffffffffu, deg);
           double2 acc_f = zero2, acc_s = zero2;
-          tile_hops<NC>(rq, max_deg, x_first, x_second, a.coef, acc_f, acc_s);
+          tile_hops<NC>(hd.rq, max_deg, x_first, x_second, a.coef, acc_f, acc_s);
           if (active) {  // diagonal: own row of the shared tile
             const double2 oa = *reinterpret_cast<const double2*>(x_first + (size_t)pos * 128);
             const double2 ob = *reinterpret_cast<const double2*>(x_second + (size_t)pos * 128);
-            acc_f.x = fma(dg, oa.x, acc_f.x);
-            acc_f.y = fma(dg, oa.y, acc_f.y);
-            acc_s.x = fma(dg, ob.x, acc_s.x);
-            acc_s.y = fma(dg, ob.y, acc_s.y);
+            acc_f.x = fma(hd.dg, oa.x, acc_f.x);
+            acc_f.y = fma(hd.dg, oa.y, acc_f.y);
+            acc_s.x = fma(hd.dg, ob.x, acc_s.x);
+            acc_s.y = fma(hd.dg, ob.y, acc_s.y);
           }
           D4 acc = to_lohi(acc_f, acc_s, odd);
+          d4_fma(signed_coef(a.ccoef[(hd.side.y >> kCrossPosBits) & 15u], hd.side.y), g0, acc);
+          d4_fma(signed_coef(a.ccoef[(hd.side.z >> kCrossPosBits) & 15u], hd.side.z), g1, acc);
+          d4_fma(signed_coef(a.ccoef[(hd.side.w >> kCrossPosBits) & 15u], hd.side.w), g2, acc);
+          if (a.side_words > 4 && active) {  // cross-cut words 3..6 (wide cuts only)
+            const uint4 more = __ldg(reinterpret_cast<const uint4*>(side + (size_t)pos * 8 + 4));
+            const uint32_t cw[4] = {more.x, more.y, more.z, more.w};
 #pragma unroll
-          for (int j = 0; j < kTileMaxCross; ++j)  // hops across the cut: other tiles, from L2
-            if (cc[j] >= 0) {
-              const D4 g = ldg256(X1 + (size_t)cc[j] * kTilePanel + 4 * q);
-              acc.x = fma(cv[j], g.x, acc.x);
-              acc.y = fma(cv[j], g.y, acc.y);
-              acc.z = fma(cv[j], g.z, acc.z);
-              acc.w = fma(cv[j], g.w, acc.w);
-            }
+            for (int j = 0; j < 4; ++j)
+              if (cw[j] != kCrossNone) {
+                const D4 g = ldg256(X1 + (size_t)(cw[j] & kCrossPosMask) * kTilePanel + 4 * q);
+                d4_fma(signed_coef(a.ccoef[(cw[j] >> kCrossPosBits) & 15u], cw[j]), g, acc);
+              }
+          }
+          D4 b;
           b.x = fma(a.pf, acc.x, pk.x);
           b.y = fma(a.pf, acc.y, pk.y);
           b.z = fma(a.pf, acc.z, pk.z);
           b.w = fma(a.pf, acc.w, pk.w);
-        }
-        if (active) {
-          if (a.mode == MODE_LAST) {
-            stg256_stream(a.W + (size_t)dst * a.w_ld + panel * kTilePanel + 4 * q, b);
-          } else {
-            stg256_stream(Bout + (size_t)dst * kTilePanel + 4 * q, b);
-            stg256(scratch + (size_t)pos * kTilePanel + 4 * q, b);
+          if (active) {
+            if (MODE == MODE_LAST) {
+              stg256_hint(a.W + (size_t)dst * a.w_ld + panel * kTilePanel + 4 * q, b, pol_first);
+            } else {
+              stg256_hint(Bout + (size_t)dst * kTilePanel + 4 * q, b, pol_first);
+              stg256_hint(scratch + (size_t)pos * kTilePanel + 4 * q, b, pol_last);
+            }
           }
         }
       }
-      if (a.mode == MODE_LAST) {
+      if (MODE == MODE_LAST) {
         __syncthreads();  // the next bulk copy overwrites the tile
         continue;
       }
 
       // ---- b_k becomes the shared tile ------------------------------------------------------
-      if (first_pos < nrows) rq_next = __ldg(rec + (size_t)first_pos * 4 + q);
+      uint4 rq_n = make_uint4(0u, 0u, 0u, 0u);
+      if (first_pos < nrows) rq_n = __ldg(rec + (size_t)first_pos * 4 + q);
       __threadfence_block();
       fence_proxy_async();
       __syncthreads();
-      if (tid == 0) tile_load(smem_raw, scratch, (unsigned)nrows * 128u, &bar);
+      if (tid == 0) tile_load(smem_raw, scratch, (unsigned)nrows * 128u, &bar, pol_last);
       mbar_wait(&bar, parity);
       parity ^= 1u;
 
       // ---- phase 3: P_{k-1} = c_{k-1} V + p_{k-1} O_l b_k + q_{k-1} b_k + r b_{k+1} ------------
-      for (int base = warp * kRowsPerIter; base < nrows; base += kWarps * kRowsPerIter) {
+      for (int base = warp * kRowsPerIter; base < nrows; base += kIterRows) {
         const int pos = base + slot;
         const bool active = pos < nrows;
-        const size_t row = (size_t)row0 + pos;
-        const uint4 rq = rq_next;
+        const uint4 rq = rq_n;
         {
-          const int pos_n = pos + kWarps * kRowsPerIter;
-          if (pos_n < nrows) rq_next = __ldg(rec + (size_t)pos_n * 4 + q);
+          const int pos_n = pos + kIterRows;
+          rq_n = make_uint4(0u, 0u, 0u, 0u);
+          if (pos_n < nrows) rq_n = __ldg(rec + (size_t)pos_n * 4 + q);
         }
         D4 x1, v;
-        x1.x = x1.y = x1.z = x1.w = 0.0;
-        v = x1;
+        d4_zero(x1);
+        d4_zero(v);
         int dst = 0;
         if (active) {
-          dst = __ldg(a.dst_map + row);
-          if (a.rs != 0.0) x1 = ldg256(X1 + row * kTilePanel + 4 * q);
-          if (a.cs != 0.0) v = ldg256_stream(V + row * kTilePanel + 4 * q);
+          dst = __ldg(dst_map + pos);
+          if (a.rs != 0.0) x1 = ldg256(X1 + ((size_t)row0 + pos) * kTilePanel + 4 * q);
+          if (a.cs != 0.0) v = ldg256_stream(V + (size_t)pos * kTilePanel + 4 * q, pol_first);
         }
         const int deg = __shfl_sync(0xffffffffu, (int)rq.x, 0, 4);
-        const int max_deg = __reduce_max_sync(0xffffffffu, active ? deg : 0);
+        const int max_deg = __reduce_max_sync(0xffffffffu, deg);
         double2 acc_f = zero2, acc_s = zero2;
         tile_hops<NC>(rq, max_deg, x_first, x_second, a.coef, acc_f, acc_s);
         if (active) {
@@ -349,7 +413,7 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
           y.y = fma(a.cs, v.y, fma(a.rs, x1.y, y.y));
           y.z = fma(a.cs, v.z, fma(a.rs, x1.z, y.z));
           y.w = fma(a.cs, v.w, fma(a.rs, x1.w, y.w));
-          stg256_stream(Pout + (size_t)dst * kTilePanel + 4 * q, y);
+          stg256_hint(Pout + (size_t)dst * kTilePanel + 4 * q, y, pol_first);
         }
       }
       __syncthreads();  // all reads of the tile done before the next bulk copy
@@ -369,7 +433,7 @@ __global__ void __launch_bounds__(256) tiled_pack_kernel(long long n, int n_pane
   const long long row = t / per_row;
   if (row >= n) return;
   const int w = (int)(t % per_row), panel = w >> 2, piece = w & 3;
-  const D4 v = ldg256_stream(V + t * 4);
+  const D4 v = ldg256_plain_stream(V + t * 4);
   const size_t ps = (size_t)n * kTilePanel;
   stg256(V0 + panel * ps + (size_t)__ldg(from_nat0 + row) * kTilePanel + 4 * piece, v);
   stg256(V1 + panel * ps + (size_t)__ldg(from_nat1 + row) * kTilePanel + 4 * piece, v);
@@ -377,7 +441,12 @@ __global__ void __launch_bounds__(256) tiled_pack_kernel(long long n, int n_pane
 
 template <int NC>
 int launch_sweep(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
-  tiled_sweep_kernel<NC><<<p->grid, kTileThreads, p->smem_bytes, st>>>(a);
+  if (a.mode == MODE_INIT)
+    tiled_sweep_kernel<NC, MODE_INIT><<<p->grid, kTileThreads, p->smem_bytes, st>>>(a);
+  else if (a.mode == MODE_LAST)
+    tiled_sweep_kernel<NC, MODE_LAST><<<p->grid, kTileThreads, p->smem_bytes, st>>>(a);
+  else
+    tiled_sweep_kernel<NC, MODE_STEP><<<p->grid, kTileThreads, p->smem_bytes, st>>>(a);
   POLFED_LAUNCH_CHECK("tiled_sweep_kernel");
   return POLFED_OK;
 }
@@ -386,22 +455,22 @@ int sweep(const TiledPlan* p, int layout, SweepArgs a, cudaStream_t st) {
   const TiledLayout& L = p->lay[layout];
   a.records = L.d_records;
   a.diag = L.d_diag;
-  a.cc_col = L.d_cc_col;
-  a.cc_val = L.d_cc_val;
-  a.n_cross = L.n_cross;
+  a.side = L.d_side;
+  a.side_words = L.side_words;
+  for (int c = 0; c <= kTileMaxCrossCoef; ++c) a.ccoef[c] = L.ccoef[c];
   a.dst_map = (a.mode == MODE_LAST) ? L.d_to_natural : L.d_to_other;
   for (int c = 0; c < kTileMaxCoef; ++c) a.coef[c] = L.coef[c];
   POLFED_CUDA(cudaMemsetAsync(p->d_counter, 0, sizeof(int), st));
   return L.n_coef <= 2 ? launch_sweep<2>(p, a, st) : launch_sweep<4>(p, a, st);
 }
 
-template <int NC>
+template <int NC, int MODE>
 int configure_one(TiledPlan* p, int* occ) {
-  POLFED_CUDA(cudaFuncSetAttribute(tiled_sweep_kernel<NC>,
+  POLFED_CUDA(cudaFuncSetAttribute(tiled_sweep_kernel<NC, MODE>,
                                    cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)p->smem_bytes));
   int o = 0;
-  POLFED_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, tiled_sweep_kernel<NC>,
+  POLFED_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, tiled_sweep_kernel<NC, MODE>,
                                                             kTileThreads, p->smem_bytes));
   if (o < 1) return fail(POLFED_ECUDA, "tiled format: sweep kernel does not fit an SM");
   *occ = (*occ == 0 || o < *occ) ? o : *occ;
@@ -413,8 +482,12 @@ int configure_one(TiledPlan* p, int* occ) {
 int tiled_configure_launch(TiledPlan* p) {
   p->smem_bytes = (size_t)(p->max_tile_rows + 1) * 128;  // + the zero row
   int occ = 0, rc;
-  if ((rc = configure_one<2>(p, &occ))) return rc;
-  if ((rc = configure_one<4>(p, &occ))) return rc;
+  if ((rc = configure_one<2, MODE_STEP>(p, &occ))) return rc;
+  if ((rc = configure_one<2, MODE_INIT>(p, &occ))) return rc;
+  if ((rc = configure_one<2, MODE_LAST>(p, &occ))) return rc;
+  if ((rc = configure_one<4, MODE_STEP>(p, &occ))) return rc;
+  if ((rc = configure_one<4, MODE_INIT>(p, &occ))) return rc;
+  if ((rc = configure_one<4, MODE_LAST>(p, &occ))) return rc;
   int dev = 0, sms = 148;
   POLFED_CUDA(cudaGetDevice(&dev));
   POLFED_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
