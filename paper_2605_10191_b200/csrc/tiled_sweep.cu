@@ -239,30 +239,62 @@ __device__ __forceinline__ RowHead load_head(const uint4* rec, const uint32_t* s
   return h;
 }
 
+// A warp claims the next kRowsPerIter positions of the tile (rows are sorted by falling degree,
+// so claiming in order also balances the warps).
+__device__ __forceinline__ int grab_chunk(int* counter, int lane) {
+  int v = 0;
+  if (lane == 0) v = atomicAdd(counter, kRowsPerIter);
+  return __shfl_sync(0xffffffffu, v, 0);
+}
+
+// Ask L2 for the tile panel of b_{k+1} this CTA loads next, while phase 3 of the current one runs.
+__device__ __forceinline__ void next_tile_prefetch(const SweepArgs& a, int tile, int tile_n,
+                                                   int panel, size_t panel_stride, int tid) {
+  int npanel = panel + 1;
+  if (npanel == a.n_panels) {
+    tile = tile_n;
+    npanel = 0;
+  }
+  if (tile >= a.n_tiles) return;
+  const int row0 = __ldg(a.tile_row0 + tile);
+  const unsigned bytes = (unsigned)(__ldg(a.tile_row0 + tile + 1) - row0) * 128u;
+  const unsigned at = (unsigned)tid * 2048u;
+  if (at < bytes)
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(
+                     a.X1 + npanel * panel_stride + (size_t)row0 * kTilePanel + at / 8),
+                 "r"(min(2048u, bytes - at))
+                 : "memory");
+}
+
 template <int NC, int MODE>
 __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const SweepArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];  // (max_tile_rows + 1) x 128 B
   __shared__ uint64_t bar;
-  __shared__ int s_tile;
+  __shared__ int s_tile[2];
+  __shared__ int s_chunk[2];  // next unclaimed position of the running phase / the one after it
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int q = lane & 3, slot = lane >> 2;
   const bool odd = slot & 1;
   const unsigned char* x_first = smem_raw + 32 * q + (odd ? 16 : 0);
   const unsigned char* x_second = smem_raw + 32 * q + (odd ? 0 : 16);
-  if (tid == 0) mbar_init(&bar, 1);
+  if (tid == 0) {
+    mbar_init(&bar, 1);
+    s_tile[0] = atomicAdd(a.counter, 1);
+    s_chunk[0] = s_chunk[1] = 0;
+  }
   __syncthreads();
   unsigned parity = 0;
+  int phase = 0;  // selects the chunk counter; the other one is reset at the start of a phase
   double* scratch = a.scratch + (size_t)blockIdx.x * a.max_tile_rows * kTilePanel;
   const size_t panel_stride = (size_t)a.n * kTilePanel;  // doubles per panel
   const double2 zero2 = make_double2(0.0, 0.0);
   const int first_pos = warp * kRowsPerIter + slot;
   const uint64_t pol_first = l2_policy_evict_first(), pol_last = l2_policy_evict_last();
 
-  for (;;) {
-    if (tid == 0) s_tile = atomicAdd(a.counter, 1);
-    __syncthreads();
-    const int tile = s_tile;
+  for (int it = 0;; ++it) {
+    const int tile = s_tile[it & 1];
     if (tile >= a.n_tiles) break;
+    if (tid == 0) s_tile[(it + 1) & 1] = atomicAdd(a.counter, 1);  // read after later barriers
     const int row0 = __ldg(a.tile_row0 + tile);
     const int nrows = __ldg(a.tile_row0 + tile + 1) - row0;
     const uint4* rec = reinterpret_cast<const uint4*>(a.records) +
@@ -297,14 +329,18 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
         if (tid == 0)
           tile_load(smem_raw, X1 + (size_t)row0 * kTilePanel, (unsigned)nrows * 128u, &bar,
                     pol_last);
-        RowHead nx = load_head(rec, side, a.side_words, diag, first_pos, nrows, q);
+        if (tid == 0) s_chunk[(phase + 1) & 1] = 0;
+        int* const chunk = &s_chunk[phase & 1];
+        ++phase;
+        int base = grab_chunk(chunk, lane), base_n = grab_chunk(chunk, lane);
+        RowHead nx = load_head(rec, side, a.side_words, diag, base + slot, nrows, q);
         mbar_wait(&bar, parity);
         parity ^= 1u;
-        for (int base = warp * kRowsPerIter; base < nrows; base += kIterRows) {
+        for (; base < nrows; base = base_n, base_n = grab_chunk(chunk, lane)) {
           const int pos = base + slot;
           const bool active = pos < nrows;
           const RowHead hd = nx;
-          nx = load_head(rec, side, a.side_words, diag, pos + kIterRows, nrows, q);
+          nx = load_head(rec, side, a.side_words, diag, base_n + slot, nrows, q);
           // this row's stream and the cross-cut rows (other tiles, from L2) fly during the hops
           D4 pk, g0, g1, g2;
           d4_zero(pk);
@@ -369,22 +405,30 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
       }
 
       // ---- b_k becomes the shared tile ------------------------------------------------------
-      uint4 rq_n = make_uint4(0u, 0u, 0u, 0u);
-      if (first_pos < nrows) rq_n = __ldg(rec + (size_t)first_pos * 4 + q);
       __threadfence_block();
       fence_proxy_async();
       __syncthreads();
-      if (tid == 0) tile_load(smem_raw, scratch, (unsigned)nrows * 128u, &bar, pol_last);
+      if (tid == 0) {
+        tile_load(smem_raw, scratch, (unsigned)nrows * 128u, &bar, pol_last);
+        s_chunk[(phase + 1) & 1] = 0;
+      }
+      int* const chunk = &s_chunk[phase & 1];
+      ++phase;
+      int base = grab_chunk(chunk, lane), base_n = grab_chunk(chunk, lane);
+      uint4 rq_n = make_uint4(0u, 0u, 0u, 0u);
+      if (base + slot < nrows) rq_n = __ldg(rec + (size_t)(base + slot) * 4 + q);
+      if (MODE == MODE_STEP)
+        next_tile_prefetch(a, tile, s_tile[(it + 1) & 1], panel, panel_stride, tid);
       mbar_wait(&bar, parity);
       parity ^= 1u;
 
       // ---- phase 3: P_{k-1} = c_{k-1} V + p_{k-1} O_l b_k + q_{k-1} b_k + r b_{k+1} ------------
-      for (int base = warp * kRowsPerIter; base < nrows; base += kIterRows) {
+      for (; base < nrows; base = base_n, base_n = grab_chunk(chunk, lane)) {
         const int pos = base + slot;
         const bool active = pos < nrows;
         const uint4 rq = rq_n;
         {
-          const int pos_n = pos + kIterRows;
+          const int pos_n = base_n + slot;
           rq_n = make_uint4(0u, 0u, 0u, 0u);
           if (pos_n < nrows) rq_n = __ldg(rec + (size_t)pos_n * 4 + q);
         }
