@@ -41,7 +41,10 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
-    cmd = [_nvcc(), *NVCC_FLAGS, "-I", os.path.join(ROOT, "include"), "-I", CSRC,
+    # POLFED_NVCC_EXTRA: extra nvcc flags for developer builds, e.g. -DPOLFED_TILED_PROFILE
+    # (per-phase cycle counters of the tiled sweep, profiles/r01_tiled_phase_ablation.md)
+    extra = os.environ.get("POLFED_NVCC_EXTRA", "").split()
+    cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-I", os.path.join(ROOT, "include"), "-I", CSRC,
            "-o", LIB, *sources(), "-lcusolver"]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")

@@ -9,6 +9,8 @@
 // shared memory the same 32 bytes are read as two 16-byte chunks; the rows a warp works on
 // alternate the order of the two (even row slots low chunk first, odd slots high chunk first),
 // so that the two rows of a quarter-warp always hit disjoint banks whatever rows they gather.
+#include <cstdlib>
+
 #include "tiled.cuh"
 
 namespace polfed {
@@ -44,6 +46,24 @@ struct SweepArgs {
   double pf;              // finishing scalar p_k
   double ps, qs, rs, cs;  // starting scalars of step k-1
   int mode;
+#ifdef POLFED_TILED_PROFILE
+  int skip;                  // POLFED_TILED_SKIP: parts of the sweep left out (timing only)
+  unsigned long long* prof;  // per CTA: cycles in tile load / phase 2 / reload / phase 3, count
+#endif
+};
+
+// Developer build (-DPOLFED_TILED_PROFILE, see build.py): per-phase cycle counters and a mask that
+// leaves parts of the sweep out, for the ablation in profiles/r01_tiled_phase_ablation.md.
+#ifdef POLFED_TILED_PROFILE
+#define PROF_SKIP(bit) ((a.skip & (bit)) != 0)
+#define PROF_CLOCK(var) var = clock64()
+#else
+#define PROF_SKIP(bit) false
+#define PROF_CLOCK(var)
+#endif
+enum {
+  SKIP_HOPS2 = 1, SKIP_HOPS3 = 2, SKIP_PK = 4, SKIP_CROSS = 8, SKIP_BOUT = 16, SKIP_SCRATCH = 32,
+  SKIP_X1 = 64, SKIP_V = 128, SKIP_POUT = 256
 };
 
 struct D4 {
@@ -174,23 +194,60 @@ __device__ __forceinline__ void hop_fma(uint32_t cls, uint32_t sg, uint32_t off,
   acc_s.y = fma(cf, xb.y, acc_s.y);
 }
 
+// One record word = two neighbours: the quad shuffle of the word and its four 16-byte gathers.
+struct HopWord {
+  uint32_t word;
+  double2 a0, a1, b0, b1;  // neighbour A (first, second chunk), neighbour B
+};
+
+__device__ __forceinline__ HopWord hop_fetch(const uint4 rq, int w,
+                                             const unsigned char* __restrict__ x_first,
+                                             const unsigned char* __restrict__ x_second) {
+  const uint32_t mine = (w & 3) == 0 ? rq.x : (w & 3) == 1 ? rq.y : (w & 3) == 2 ? rq.z : rq.w;
+  HopWord h;
+  h.word = __shfl_sync(0xffffffffu, mine, w >> 2, 4);
+  const uint32_t oa = h.word & 0x3ff80u, ob = (h.word >> 11) & 0x3ff80u;
+  h.a0 = *reinterpret_cast<const double2*>(x_first + oa);
+  h.a1 = *reinterpret_cast<const double2*>(x_second + oa);
+  h.b0 = *reinterpret_cast<const double2*>(x_first + ob);
+  h.b1 = *reinterpret_cast<const double2*>(x_second + ob);
+  return h;
+}
+
+template <int NC>
+__device__ __forceinline__ void hop_apply(const HopWord& h, const double (&coef)[kTileMaxCoef],
+                                          double2& acc_f, double2& acc_s) {
+  const double ca = signed_coef(pick_coef<NC>(h.word & 3u, coef), h.word << 1);
+  const double cb = signed_coef(pick_coef<NC>((h.word >> 2) & 3u, coef), h.word);
+  acc_f.x = fma(ca, h.a0.x, acc_f.x);
+  acc_f.y = fma(ca, h.a0.y, acc_f.y);
+  acc_s.x = fma(ca, h.a1.x, acc_s.x);
+  acc_s.y = fma(ca, h.a1.y, acc_s.y);
+  acc_f.x = fma(cb, h.b0.x, acc_f.x);
+  acc_f.y = fma(cb, h.b0.y, acc_f.y);
+  acc_s.x = fma(cb, h.b1.x, acc_s.x);
+  acc_s.y = fma(cb, h.b1.y, acc_s.y);
+}
+
 // All in-tile neighbours of the row whose record quarter this lane holds (rq); max_deg is
-// warp-uniform, shorter rows run into entries that point at the zero row.
+// warp-uniform, shorter rows run into entries that point at the zero row.  The gathers of word
+// w + 1 are issued before the FMAs of word w.
 template <int NC>
 __device__ __forceinline__ void tile_hops(const uint4 rq, int max_deg,
                                           const unsigned char* __restrict__ x_first,
                                           const unsigned char* __restrict__ x_second,
                                           const double (&coef)[kTileMaxCoef], double2& acc_f,
                                           double2& acc_s) {
+  if (max_deg <= 0) return;
+  HopWord cur = hop_fetch(rq, 1, x_first, x_second);
 #pragma unroll
   for (int w = 1; w <= kTileMaxDeg / 2; ++w) {
-    if (2 * (w - 1) >= max_deg) break;
-    const uint32_t mine = (w & 3) == 0 ? rq.x : (w & 3) == 1 ? rq.y : (w & 3) == 2 ? rq.z : rq.w;
-    const uint32_t word = __shfl_sync(0xffffffffu, mine, w >> 2, 4);
-    hop_fma<NC>(word & 3u, word << 1, word & 0x3ff80u, x_first, x_second, coef, acc_f, acc_s);
-    if (2 * w - 1 < max_deg)  // an odd warp-wide degree ends on a half-used word
-      hop_fma<NC>((word >> 2) & 3u, word, (word >> 11) & 0x3ff80u, x_first, x_second, coef, acc_f,
-                  acc_s);
+    HopWord nxt = cur;
+    const bool more = w < kTileMaxDeg / 2 && 2 * w < max_deg;
+    if (more) nxt = hop_fetch(rq, w + 1, x_first, x_second);
+    hop_apply<NC>(cur, coef, acc_f, acc_s);
+    if (!more) break;
+    cur = nxt;
   }
 }
 
@@ -306,6 +363,9 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
     __syncthreads();
 
     for (int panel = 0; panel < a.n_panels; ++panel) {
+#ifdef POLFED_TILED_PROFILE
+      long long t0 = clock64(), t1 = t0, t2 = t0, t3 = t0, t4 = t0;
+#endif
       const double* X1 = a.X1 + panel * panel_stride;
       const double* Pk = a.Pk + panel * panel_stride + (size_t)row0 * kTilePanel;
       const double* V = a.V + panel * panel_stride + (size_t)row0 * kTilePanel;
@@ -336,6 +396,7 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
         RowHead nx = load_head(rec, side, a.side_words, diag, base + slot, nrows, q);
         mbar_wait(&bar, parity);
         parity ^= 1u;
+        PROF_CLOCK(t1);
         for (; base < nrows; base = base_n, base_n = grab_chunk(chunk, lane)) {
           const int pos = base + slot;
           const bool active = pos < nrows;
@@ -349,17 +410,17 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
           d4_zero(g2);
           int dst = (int)hd.side.x;
           if (active) {
-            pk = ldg256_stream(Pk + (size_t)pos * kTilePanel + 4 * q, pol_first);
+            if (!PROF_SKIP(SKIP_PK)) pk = ldg256_stream(Pk + (size_t)pos * kTilePanel + 4 * q, pol_first);
             if (MODE == MODE_LAST) dst = __ldg(dst_map + pos);
           }
-          if (hd.side.y != kCrossNone)
+          if (hd.side.y != kCrossNone && !PROF_SKIP(SKIP_CROSS))
             g0 = ldg256(X1 + (size_t)(hd.side.y & kCrossPosMask) * kTilePanel + 4 * q);
-          if (hd.side.z != kCrossNone)
+          if (hd.side.z != kCrossNone && !PROF_SKIP(SKIP_CROSS))
             g1 = ldg256(X1 + (size_t)(hd.side.z & kCrossPosMask) * kTilePanel + 4 * q);
-          if (hd.side.w != kCrossNone)
+          if (hd.side.w != kCrossNone && !PROF_SKIP(SKIP_CROSS))
             g2 = ldg256(X1 + (size_t)(hd.side.w & kCrossPosMask) * kTilePanel + 4 * q);
           const int deg = __shfl_sync(0xffffffffu, (int)hd.rq.x, 0, 4);
-          const int max_deg = __reduce_max_sync(0xffffffffu, deg);
+          const int max_deg = PROF_SKIP(SKIP_HOPS2) ? 0 : __reduce_max_sync(0xffffffffu, deg);
           double2 acc_f = zero2, acc_s = zero2;
           tile_hops<NC>(hd.rq, max_deg, x_first, x_second, a.coef, acc_f, acc_s);
           if (active) {  // diagonal: own row of the shared tile
@@ -393,8 +454,8 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
             if (MODE == MODE_LAST) {
               stg256_hint(a.W + (size_t)dst * a.w_ld + panel * kTilePanel + 4 * q, b, pol_first);
             } else {
-              stg256_hint(Bout + (size_t)dst * kTilePanel + 4 * q, b, pol_first);
-              stg256_hint(scratch + (size_t)pos * kTilePanel + 4 * q, b, pol_last);
+              if (!PROF_SKIP(SKIP_BOUT)) stg256_hint(Bout + (size_t)dst * kTilePanel + 4 * q, b, pol_first);
+              if (!PROF_SKIP(SKIP_SCRATCH)) stg256_hint(scratch + (size_t)pos * kTilePanel + 4 * q, b, pol_last);
             }
           }
         }
@@ -408,6 +469,7 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
       __threadfence_block();
       fence_proxy_async();
       __syncthreads();
+      PROF_CLOCK(t2);
       if (tid == 0) {
         tile_load(smem_raw, scratch, (unsigned)nrows * 128u, &bar, pol_last);
         s_chunk[(phase + 1) & 1] = 0;
@@ -421,6 +483,10 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
         next_tile_prefetch(a, tile, s_tile[(it + 1) & 1], panel, panel_stride, tid);
       mbar_wait(&bar, parity);
       parity ^= 1u;
+      PROF_CLOCK(t3);
+      // the parked copy is dead once it is back in shared memory: drop it from L2 unwritten
+      for (int r = tid; r < nrows; r += kTileThreads)
+        asm volatile("discard.global.L2 [%0], 128;" ::"l"(scratch + (size_t)r * kTilePanel) : "memory");
 
       // ---- phase 3: P_{k-1} = c_{k-1} V + p_{k-1} O_l b_k + q_{k-1} b_k + r b_{k+1} ------------
       for (; base < nrows; base = base_n, base_n = grab_chunk(chunk, lane)) {
@@ -438,11 +504,11 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
         int dst = 0;
         if (active) {
           dst = __ldg(dst_map + pos);
-          if (a.rs != 0.0) x1 = ldg256(X1 + ((size_t)row0 + pos) * kTilePanel + 4 * q);
-          if (a.cs != 0.0) v = ldg256_stream(V + (size_t)pos * kTilePanel + 4 * q, pol_first);
+          if (a.rs != 0.0 && !PROF_SKIP(SKIP_X1)) x1 = ldg256(X1 + ((size_t)row0 + pos) * kTilePanel + 4 * q);
+          if (a.cs != 0.0 && !PROF_SKIP(SKIP_V)) v = ldg256_stream(V + (size_t)pos * kTilePanel + 4 * q, pol_first);
         }
         const int deg = __shfl_sync(0xffffffffu, (int)rq.x, 0, 4);
-        const int max_deg = __reduce_max_sync(0xffffffffu, deg);
+        const int max_deg = PROF_SKIP(SKIP_HOPS3) ? 0 : __reduce_max_sync(0xffffffffu, deg);
         double2 acc_f = zero2, acc_s = zero2;
         tile_hops<NC>(rq, max_deg, x_first, x_second, a.coef, acc_f, acc_s);
         if (active) {
@@ -457,10 +523,22 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
           y.y = fma(a.cs, v.y, fma(a.rs, x1.y, y.y));
           y.z = fma(a.cs, v.z, fma(a.rs, x1.z, y.z));
           y.w = fma(a.cs, v.w, fma(a.rs, x1.w, y.w));
-          stg256_hint(Pout + (size_t)dst * kTilePanel + 4 * q, y, pol_first);
+          if (!PROF_SKIP(SKIP_POUT)) stg256_hint(Pout + (size_t)dst * kTilePanel + 4 * q, y, pol_first);
         }
       }
       __syncthreads();  // all reads of the tile done before the next bulk copy
+#ifdef POLFED_TILED_PROFILE
+      t4 = clock64();
+      if (tid == 0 && a.prof) {
+        unsigned long long* pr = a.prof + blockIdx.x * 8;
+        pr[0] += t1 - t0;
+        pr[1] += t2 - t1;
+        pr[2] += t3 - t2;
+        pr[3] += t4 - t3;
+        pr[4] += 1;
+        pr[5] += nrows;
+      }
+#endif
     }
   }
 }
@@ -569,6 +647,16 @@ int tiled_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
   POLFED_LAUNCH_CHECK("tiled_pack_kernel");
 
   SweepArgs a{};
+#ifdef POLFED_TILED_PROFILE
+  static unsigned long long* d_prof = nullptr;
+  {
+    const char* e = getenv("POLFED_TILED_SKIP");
+    a.skip = e ? atoi(e) : 0;
+    if (!d_prof) POLFED_CUDA(cudaMalloc(&d_prof, sizeof(unsigned long long) * 8 * 1024));
+    POLFED_CUDA(cudaMemsetAsync(d_prof, 0, sizeof(unsigned long long) * 8 * 1024, st));
+    a.prof = d_prof;
+  }
+#endif
   a.n = ham->n;
   a.n_tiles = p->n_tiles;
   a.n_panels = n_panels;
@@ -603,6 +691,20 @@ int tiled_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
     int rc = sweep(p, layout, a, st);
     if (rc) return rc;
   }
+#ifdef POLFED_TILED_PROFILE
+  {
+    static unsigned long long h[8 * 1024];
+    POLFED_CUDA(cudaStreamSynchronize(st));
+    POLFED_CUDA(cudaMemcpy(h, d_prof, sizeof(h), cudaMemcpyDeviceToHost));
+    double t[6] = {0, 0, 0, 0, 0, 0};
+    for (int b = 0; b < p->grid && b < 1024; ++b)
+      for (int i = 0; i < 6; ++i) t[i] += (double)h[b * 8 + i];
+    fprintf(stderr,
+            "tiled profile: skip=%d K=%d tile-panels=%.0f rows/tile-panel=%.1f cycles/tile-panel: "
+            "load %.0f phase2 %.0f reload %.0f phase3 %.0f\n",
+            a.skip, K, t[4], t[5] / t[4], t[0] / t[4], t[1] / t[4], t[2] / t[4], t[3] / t[4]);
+  }
+#endif
   return POLFED_OK;
 }
 
