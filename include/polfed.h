@@ -119,10 +119,12 @@ int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_ter
  * n_sites - m bits (m = ceil(n_sites/2)) are one tile; hops among the low m sites stay inside it
  * and are stored once per particle-number class as neighbour index + sign, grouped by the at
  * most 4 distinct |amp| values; hops among the high sites are tile-local in the site-reversed
- * row order; the diagonal and the few hops across the cut stay a small CSR.
+ * row order; the diagonal and the few hops across the cut are kept per row (at most 7 such hops
+ * per state, at most 15 distinct |amp| among them; one packed 32-bit word each).
  * polfed_filter_apply then runs the recurrence as sweeps that alternate between the two row
  * orders with the tile held in shared memory (same result up to rounding order).
- * Requirements (else POLFED_EINVAL): fixed-n_up basis, 4 <= n_sites <= 26, no dense block,
+ * Requirements (else POLFED_EINVAL): fixed-n_up basis of fewer than 2^26 states,
+ * 4 <= n_sites <= 26, no dense block,
  * off-diagonal terms of kind EXCH or HOPJW only, at most 4 distinct |amp| and 24 hops per state
  * inside a tile.  Used by polfed_filter_apply for s in {16, 32}; every other entry point uses
  * the CSR. */
