@@ -132,3 +132,79 @@ def test_tiled_handle_still_serves_csr_entry_points(P):
     work = torch.empty(2 * H.n * 4, dtype=torch.float64, device="cuda")
     P.polfed_filter_apply(ham, 0.0, 20.0, coeffs, 4, dev(V), W, work)
     assert rel_l2(W.cpu().numpy(), core.clenshaw(H, 0.0, 20.0, coeffs, V)) <= 1e-12
+
+
+# ---- full BASELINE sizes, in the launch configuration bench.py times --------------------------
+
+def test_tiled_full_size_config3_matches_oracle(P):
+    """Config 3 (XXZ L=20, D=184 756, s=16): the whole filter against the oracle, small K."""
+    w = workloads.make_workload(3)
+    _, H = core.hamiltonian(w)
+    V = workloads.start_block(H.n, w.s, seed=2003)
+    coeffs = np.random.default_rng(33).standard_normal(8)
+    a, b = -0.4, 1.05 * gershgorin(H)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    got = tiled_filter(P, build(P, w.n_sites, w.n_up, w.terms), a, b, coeffs, V)
+    assert rel_l2(got, want) <= 1e-12
+
+
+def _closure(states, rows, w):
+    """Sorted rows plus every column their matrix rows touch, and the mini-CSR of `rows`."""
+    mini = core.build_csr_rows(states, rows, w.terms, w.dot_bits, w.dot_dense)
+    return np.unique(np.concatenate([rows, mini.col.astype(np.int64)])), mini
+
+
+def test_tiled_full_size_config5_sampled_rows(P):
+    """Config 5 (D=10 400 600, s=32), K=3: first, two recurrence and last sweep of the tiled
+    pipeline.  The oracle follows Eq. (51) on the rows that the sampled outputs depend on
+    (two levels of matrix neighbours), one row at a time through its own CSR builder and SpMM;
+    entries outside that set are NaN, so a wrong dependency would show."""
+    w = workloads.make_workload(5)
+    states = core.basis_states(w.n_sites, w.n_up)
+    n, s = int(states.shape[0]), w.s
+    ham = build(P, w.n_sites, w.n_up, w.terms)
+    assert ham.n == n and ham.nnz == 275_407_888
+    gen = torch.Generator(device="cuda").manual_seed(5105)
+    V = torch.randn(n, s, dtype=torch.float64, device="cuda", generator=gen)
+    a, b = 0.3, 17.0
+    c = np.array([0.7, -0.4, 0.9, 0.35])
+    need = P.polfed_filter_workspace_bytes_ham(ham, s)
+    assert need > P.polfed_filter_workspace_bytes(n, s)
+    work = torch.full((need // 8,), float("nan"), dtype=torch.float64, device="cuda")
+    W = torch.full((n, s), float("nan"), dtype=torch.float64, device="cuda")
+    P.polfed_filter_apply(ham, a, b, c, s, V, W, work)
+    torch.cuda.synchronize()
+    del work
+
+    rng = np.random.default_rng(4105)
+    R0 = np.unique(np.concatenate([[0, 1, n // 2, n - 2, n - 1], rng.integers(0, n, 150)]))
+    R1, H0 = _closure(states, R0, w)
+    R2, H1 = _closure(states, R1, w)
+    H2 = core.build_csr_rows(states, R2, w.terms, w.dot_bits, w.dot_dense)
+    Vh = V.cpu().numpy()
+
+    def scatter(rows, vals):
+        full = np.full((n, s), np.nan)
+        full[rows] = vals
+        return full
+
+    # b_3 = c_3 V everywhere; b_2 on R2; b_1 on R1; W on R0   (Eq. 50-51, R3)
+    b2 = c[2] * Vh[R2] + 2.0 * (core.spmm(H2, c[3] * Vh) - a * c[3] * Vh[R2]) / b
+    b2_full = scatter(R2, b2)
+    b1 = c[1] * Vh[R1] + 2.0 * (core.spmm(H1, b2_full) - a * b2_full[R1]) / b - c[3] * Vh[R1]
+    b1_full = scatter(R1, b1)
+    want = c[0] * Vh[R0] + (core.spmm(H0, b1_full) - a * b1_full[R0]) / b - b2_full[R0]
+    assert np.all(np.isfinite(want))
+    got = W[torch.from_numpy(R0).cuda()].cpu().numpy()
+    assert np.max(np.abs(got - want)) <= 1e-12 * max(1.0, np.abs(want).max())
+    # every output row was written, and the CSR kernel (checked row by row against the oracle in
+    # test_gpu_parity.py) gives the same block everywhere
+    assert bool(torch.isfinite(W).all())
+    work2 = torch.empty(2 * n * s, dtype=torch.float64, device="cuda")
+    B1, B2 = work2[: n * s].view(n, s), work2[n * s:].view(n, s)
+    torch.mul(V, c[3], out=B1)                                             # b_3
+    P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, 0.0, c[2], B1, None, V, B2)   # b_2
+    P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, -1.0, c[1], B2, B1, V, B1)    # b_1
+    P.polfed_fused_step(ham, s, 1.0 / b, -a / b, -1.0, c[0], B1, B2, V, B2)          # W
+    diff = float((B2 - W).norm() / W.norm())
+    assert diff <= 1e-13
