@@ -210,6 +210,27 @@ int polfed_filter_coeffs(double a, double b, double sigma, int nev, double rho_r
 int polfed_spectrum_bounds(const polfed_ham* ham, int n_steps, const double* d_v0, double margin,
                            void* stream, double* emin, double* emax, double* a, double* b);
 
+/* Kernel polynomial method, PAPER.md:310-337 (Eq. 35-39): the density of states that sizes the
+ * filter window (Eq. 40-42) when the Gaussian estimate Eq. (34) is not good enough (R7).
+ *
+ * polfed_kpm_moments: mu_m = (1/s) sum_{r<s} <r| T_m(H~) |r>, m = 0..n_moments-1 (Eq. 37-38), with
+ * H~ = (H - a)/b and T_m by the Chebyshev recurrence Eq. (28)-(30) -- one fused sparse product and
+ * one block dot product per moment.  d_R: n x s row-major fp64 DEVICE block of the random vectors
+ * |r> (iid entries of zero mean and unit variance, drawn by the caller: no RNG crosses the ABI;
+ * not modified); s in {1,2,4,8,16,32}; d_work: polfed_kpm_workspace_bytes(n, s, n_moments) bytes
+ * of DEVICE scratch, 16-byte aligned; h_moments: n_moments doubles on the HOST.  mu_0 estimates the
+ * dimension (the series integrates to it).  More than 32 vectors: call again and average.
+ * Synchronises `stream`.  Errors: POLFED_EINVAL (NULL, s, n_moments < 1, alignment),
+ * POLFED_ERANGE (b <= 0 or non-finite a, b). */
+size_t polfed_kpm_workspace_bytes(int64_t n, int s, int n_moments);
+int polfed_kpm_moments(const polfed_ham* ham, double a, double b, int n_moments, int s,
+                       const double* d_R, void* d_work, double* h_moments, void* stream);
+/* Host only: rho(E~) = [mu_0 g_0 + 2 sum_{m>=1} mu_m g_m T_m(E~)] / (pi sqrt(1 - E~^2)), Eq. (36),
+ * with the Jackson kernel g_m of Eq. (39), at n_points rescaled energies in (-1, 1) (else
+ * POLFED_ERANGE); rho is in states per unit rescaled energy, the unit polfed_filter_coeffs takes. */
+int polfed_kpm_dos(const double* h_moments, int n_moments, const double* e_rescaled, int n_points,
+                   double* rho);
+
 typedef struct {
   double tol;             /* absolute bound on ||H x - lambda x||; <= 0: 1e-8 * max(|E_min|,|E_max|) */
   int32_t max_krylov_dim; /* <= 0: 5 nev + 8 s rounded up to a multiple of s (R10), capped by n and by free memory */

@@ -12,4 +12,5 @@ from .binding import (  # noqa: F401
     polfed_filter_apply,
     polfed_filter_apply_host, polfed_filter_coeffs,
     polfed_spectrum_bounds, polfed_block_lanczos_eigs,
+    polfed_kpm_workspace_bytes, polfed_kpm_moments, polfed_kpm_dos,
 )

@@ -28,6 +28,7 @@ EXPORTS = (
     "polfed_filter_apply",
     "polfed_filter_apply_host", "polfed_filter_coeffs",
     "polfed_spectrum_bounds", "polfed_block_lanczos_eigs",
+    "polfed_kpm_workspace_bytes", "polfed_kpm_moments", "polfed_kpm_dos",
 )
 
 
@@ -102,6 +103,10 @@ def lib() -> C.CDLL:
                                          C.POINTER(f64), C.POINTER(f64)]
     L.polfed_block_lanczos_eigs.argtypes = [p, f64, i32, i32, p, C.POINTER(_Options), p, p, p,
                                             C.POINTER(_Report), p]
+    L.polfed_kpm_workspace_bytes.restype = C.c_size_t
+    L.polfed_kpm_workspace_bytes.argtypes = [i64, i32, i32]
+    L.polfed_kpm_moments.argtypes = [p, f64, f64, i32, i32, p, p, p, p]
+    L.polfed_kpm_dos.argtypes = [p, i32, p, i32, p]
     _lib = L
     return L
 
@@ -357,6 +362,39 @@ def polfed_spectrum_bounds(ham: Ham, v0, n_steps: int = 0, margin: float = -1.0,
     _check(lib().polfed_spectrum_bounds(C.c_void_p(ham.handle), n_steps, _dev(v0), margin,
                                         _stream(stream), *[C.byref(o) for o in out]))
     return tuple(o.value for o in out)
+
+
+def polfed_kpm_workspace_bytes(n: int, s: int, n_moments: int) -> int:
+    return int(lib().polfed_kpm_workspace_bytes(n, s, n_moments))
+
+
+def polfed_kpm_moments(ham: Ham, a: float, b: float, n_moments: int, R, work=None,
+                       stream=None) -> np.ndarray:
+    """Chebyshev moments mu_0..mu_{n_moments-1} of the density of states from the n x s fp64 CUDA
+    block R of random vectors (Eq. 37-38)."""
+    import torch
+    if R.dim() != 2 or R.shape[0] != ham.n:
+        raise ValueError("R must be an n x s block")
+    s = int(R.shape[1])
+    need = polfed_kpm_workspace_bytes(ham.n, s, n_moments)
+    if work is None:
+        work = torch.empty(max(need // 8, 1), dtype=torch.float64, device="cuda")
+    if work.dtype != torch.float64 or work.numel() * 8 < need:
+        raise ValueError("work is too small (polfed_kpm_workspace_bytes)")
+    out = np.empty(max(n_moments, 0), dtype=np.float64)
+    _check(lib().polfed_kpm_moments(C.c_void_p(ham.handle), a, b, n_moments, s, _block(R, ham.n, s),
+                                    _dev(work), out.ctypes.data, _stream(stream)))
+    return out
+
+
+def polfed_kpm_dos(moments: np.ndarray, e_rescaled) -> np.ndarray:
+    """Jackson-damped KPM density of states (states per unit rescaled energy), Eq. (36), (39)."""
+    mu = np.ascontiguousarray(moments, dtype=np.float64)
+    e = np.ascontiguousarray(np.atleast_1d(e_rescaled), dtype=np.float64)
+    rho = np.empty_like(e)
+    _check(lib().polfed_kpm_dos(mu.ctypes.data, mu.shape[0], e.ctypes.data, e.shape[0],
+                                rho.ctypes.data))
+    return rho
 
 
 def polfed_block_lanczos_eigs(ham: Ham, sigma: float, nev: int, s: int, V0, *, tol: float = 0.0,

@@ -133,3 +133,42 @@ def test_eigs_reports_no_convergence_and_bad_arguments(P):
     with pytest.raises(P.PolfedError) as err:
         P.polfed_block_lanczos_eigs(ham, 0.0, 4, 4, Z, a=0.0, b=20.0, K_override=20)
     assert err.value.code == P.binding.EBREAKDOWN
+
+
+@pytest.mark.parametrize("config,L_override,s", [(2, None, 8), (1, None, 1), (5, 14, 32), (4, 9, 16)])
+def test_kpm_moments_match_oracle(P, config, L_override, s):
+    """Eq. (37)-(38): Chebyshev moments from the same random block on both sides; the recurrence
+    is the fused step with c = 0, so agreement is to rounding (|T_n| <= 1 on [-1, 1])."""
+    w = workloads.make_workload(config, L_override=L_override)
+    _, H = core.hamiltonian(w)
+    v0 = workloads.start_block(H.n, 1, seed=3000 + config)[:, 0]
+    _, _, a, b = lanczos.spectrum_bounds(H, v0, m=60, margin=0.01)
+    R = np.random.default_rng(6000 + config).standard_normal((H.n, s))
+    N = 75                                                   # PAPER.md:341 (Fig. 3)
+    want = cheb.kpm_moments(H, a, b, N, R)
+    ham = build(P, w)
+    got = P.polfed_kpm_moments(ham, a, b, N, dev(R))
+    assert np.max(np.abs(got - want)) <= 1e-10 * H.n
+    assert abs(got[0] - np.sum(R * R) / s) <= 1e-10 * H.n
+    # the density integrates to mu_0 and, fed to the order rule, gives the oracle's K
+    lam = 0.1
+    rho_got = float(P.polfed_kpm_dos(got, [lam])[0])
+    rho_want = float(cheb.kpm_dos(lam, want, cheb.jackson_kernel(N))[0])
+    assert abs(rho_got - rho_want) <= 1e-9 * abs(rho_want)
+    if rho_want > 0:
+        assert abs(len(P.polfed_filter_coeffs(a, b, a + b * lam, 10, rho_got)) - 1
+                   - cheb.order_bisect(10, rho_want, lam)) <= 1
+
+
+def test_kpm_moments_argument_errors(P):
+    w = workloads.make_workload(1)
+    ham = build(P, w)
+    R = torch.randn(ham.n, 4, dtype=torch.float64, device="cuda")
+    with pytest.raises(P.PolfedError):
+        P.polfed_kpm_moments(ham, 0.0, -1.0, 10, R)          # b <= 0
+    with pytest.raises(P.PolfedError):
+        P.polfed_kpm_moments(ham, 0.0, 10.0, 0, R)           # no moments
+    with pytest.raises(P.PolfedError):
+        P.polfed_kpm_moments(ham, 0.0, 10.0, 10, torch.randn(ham.n, 3, dtype=torch.float64,
+                                                             device="cuda"))     # s = 3
+    assert P.polfed_kpm_moments(ham, 0.0, 10.0, 1, R).shape == (1,)

@@ -89,3 +89,19 @@ def test_host_argument_errors(lib):
     h = C.c_void_p()
     assert lib.polfed_ham_from_csr(-1, 0, None, None, None, C.byref(h)) == P.binding.EINVAL
     assert lib.polfed_ham_destroy(None) == 0 and lib.polfed_basis_destroy(None) == 0
+
+
+def test_kpm_dos_host_series_matches_oracle(lib):
+    """polfed_kpm_dos is host-only (Eq. 36 with the Jackson kernel Eq. 39): same numbers as the
+    oracle's series for arbitrary moments; energies outside (-1, 1) are a range error."""
+    from oracle import cheb
+    rng = np.random.default_rng(9)
+    mu = rng.standard_normal(75)
+    mu[0] = 100.0
+    e = np.linspace(-0.95, 0.95, 41)
+    want = cheb.kpm_dos(e, mu, cheb.jackson_kernel(75))
+    got = P.polfed_kpm_dos(mu, e)
+    assert np.max(np.abs(got - want)) <= 1e-11 * np.max(np.abs(want))
+    with pytest.raises(P.PolfedError):
+        P.polfed_kpm_dos(mu, [1.0])
+    assert lib.polfed_kpm_workspace_bytes(1000, 8, 75) >= (2 * 1000 * 8 + 75) * 8
