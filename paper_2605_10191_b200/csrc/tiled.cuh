@@ -38,7 +38,9 @@ constexpr int kTileMaxCrossCoef = 15; // distinct |amplitude| values among the c
 constexpr uint32_t kCrossNone = 0xffffffffu;
 constexpr int kCrossPosBits = 26;     // cross word: bits 0-25 position, 26-29 amplitude, 31 sign
 constexpr int kTilePanel = 16;        // columns per panel: 128-byte rows, conflict-free in smem
-constexpr int kTileThreads = 512;
+constexpr int kTileThreads = 512;       // one CTA per SM (tiles that fill the shared memory)
+constexpr int kTileSmallThreads = 256;  // kTileSmallCtas CTAs per SM (small tiles)
+constexpr int kTileSmallCtas = 3;
 
 // Record of one class row (position order), kTileRecWords words:
 //   word 0      in-tile degree
@@ -70,6 +72,7 @@ struct TiledPlan {
   int n_tiles = 0;
   int max_tile_rows = 0;
   int grid = 0;                     // persistent CTAs
+  int threads = kTileThreads;       // threads per CTA (kTileThreads or kTileSmallThreads)
   size_t smem_bytes = 0;
   int32_t* d_tile_row0 = nullptr;   // [n_tiles + 1]
   int32_t* d_tile_rec0 = nullptr;   // [n_tiles] first record row of the tile's class

@@ -18,7 +18,6 @@ namespace {
 
 enum { MODE_STEP = 0, MODE_INIT = 1, MODE_LAST = 2 };
 
-constexpr int kWarps = kTileThreads / 32;
 constexpr int kRowsPerIter = 8;  // rows per warp iteration
 
 struct SweepArgs {
@@ -270,7 +269,6 @@ __device__ __forceinline__ void d4_fma(double c, const D4& g, D4& acc) {
 }
 
 constexpr uint32_t kCrossPosMask = (1u << kCrossPosBits) - 1u;
-constexpr int kIterRows = kWarps * kRowsPerIter;  // rows per CTA iteration
 
 // What phase 2 needs of a row before its tile hops: the record quarter, the side record
 // (position in the other layout + first three cross-cut words) and the diagonal.  Loaded one
@@ -323,8 +321,12 @@ __device__ __forceinline__ void next_tile_prefetch(const SweepArgs& a, int tile,
                  : "memory");
 }
 
-template <int NC, int MODE>
-__global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const SweepArgs a) {
+// THREADS = 512 with one CTA per SM for tiles that fill the shared memory, 256 with three CTAs
+// per SM (85 registers) for tiles of at most a third of it.
+template <int NC, int MODE, int THREADS>
+__global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSmallCtas)
+    tiled_sweep_kernel(const SweepArgs a) {
+  constexpr int kIterRows = (THREADS / 32) * kRowsPerIter;  // rows per CTA pass (static loops)
   extern __shared__ __align__(128) unsigned char smem_raw[];  // (max_tile_rows + 1) x 128 B
   __shared__ uint64_t bar;
   __shared__ int s_tile[2];
@@ -485,7 +487,7 @@ __global__ void __launch_bounds__(kTileThreads, 1) tiled_sweep_kernel(const Swee
       parity ^= 1u;
       PROF_CLOCK(t3);
       // the parked copy is dead once it is back in shared memory: drop it from L2 unwritten
-      for (int r = tid; r < nrows; r += kTileThreads)
+      for (int r = tid; r < nrows; r += THREADS)
         asm volatile("discard.global.L2 [%0], 128;" ::"l"(scratch + (size_t)r * kTilePanel) : "memory");
 
       // ---- phase 3: P_{k-1} = c_{k-1} V + p_{k-1} O_l b_k + q_{k-1} b_k + r b_{k+1} ------------
@@ -561,16 +563,22 @@ __global__ void __launch_bounds__(256) tiled_pack_kernel(long long n, int n_pane
   stg256(V1 + panel * ps + (size_t)__ldg(from_nat1 + row) * kTilePanel + 4 * piece, v);
 }
 
-template <int NC>
-int launch_sweep(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
+template <int NC, int THREADS>
+int launch_sweep_t(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
   if (a.mode == MODE_INIT)
-    tiled_sweep_kernel<NC, MODE_INIT><<<p->grid, kTileThreads, p->smem_bytes, st>>>(a);
+    tiled_sweep_kernel<NC, MODE_INIT, THREADS><<<p->grid, THREADS, p->smem_bytes, st>>>(a);
   else if (a.mode == MODE_LAST)
-    tiled_sweep_kernel<NC, MODE_LAST><<<p->grid, kTileThreads, p->smem_bytes, st>>>(a);
+    tiled_sweep_kernel<NC, MODE_LAST, THREADS><<<p->grid, THREADS, p->smem_bytes, st>>>(a);
   else
-    tiled_sweep_kernel<NC, MODE_STEP><<<p->grid, kTileThreads, p->smem_bytes, st>>>(a);
+    tiled_sweep_kernel<NC, MODE_STEP, THREADS><<<p->grid, THREADS, p->smem_bytes, st>>>(a);
   POLFED_LAUNCH_CHECK("tiled_sweep_kernel");
   return POLFED_OK;
+}
+
+template <int NC>
+int launch_sweep(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
+  return p->threads == kTileThreads ? launch_sweep_t<NC, kTileThreads>(p, a, st)
+                                    : launch_sweep_t<NC, kTileSmallThreads>(p, a, st);
 }
 
 int sweep(const TiledPlan* p, int layout, SweepArgs a, cudaStream_t st) {
@@ -586,16 +594,28 @@ int sweep(const TiledPlan* p, int layout, SweepArgs a, cudaStream_t st) {
   return L.n_coef <= 2 ? launch_sweep<2>(p, a, st) : launch_sweep<4>(p, a, st);
 }
 
-template <int NC, int MODE>
+template <int NC, int MODE, int THREADS>
 int configure_one(TiledPlan* p, int* occ) {
-  POLFED_CUDA(cudaFuncSetAttribute(tiled_sweep_kernel<NC, MODE>,
+  POLFED_CUDA(cudaFuncSetAttribute(tiled_sweep_kernel<NC, MODE, THREADS>,
                                    cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)p->smem_bytes));
   int o = 0;
-  POLFED_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, tiled_sweep_kernel<NC, MODE>,
-                                                            kTileThreads, p->smem_bytes));
+  POLFED_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+      &o, tiled_sweep_kernel<NC, MODE, THREADS>, THREADS, p->smem_bytes));
   if (o < 1) return fail(POLFED_ECUDA, "tiled format: sweep kernel does not fit an SM");
   *occ = (*occ == 0 || o < *occ) ? o : *occ;
+  return POLFED_OK;
+}
+
+template <int THREADS>
+int configure_all(TiledPlan* p, int* occ) {
+  int rc;
+  if ((rc = configure_one<2, MODE_STEP, THREADS>(p, occ))) return rc;
+  if ((rc = configure_one<2, MODE_INIT, THREADS>(p, occ))) return rc;
+  if ((rc = configure_one<2, MODE_LAST, THREADS>(p, occ))) return rc;
+  if ((rc = configure_one<4, MODE_STEP, THREADS>(p, occ))) return rc;
+  if ((rc = configure_one<4, MODE_INIT, THREADS>(p, occ))) return rc;
+  if ((rc = configure_one<4, MODE_LAST, THREADS>(p, occ))) return rc;
   return POLFED_OK;
 }
 
@@ -604,12 +624,14 @@ int configure_one(TiledPlan* p, int* occ) {
 int tiled_configure_launch(TiledPlan* p) {
   p->smem_bytes = (size_t)(p->max_tile_rows + 1) * 128;  // + the zero row
   int occ = 0, rc;
-  if ((rc = configure_one<2, MODE_STEP>(p, &occ))) return rc;
-  if ((rc = configure_one<2, MODE_INIT>(p, &occ))) return rc;
-  if ((rc = configure_one<2, MODE_LAST>(p, &occ))) return rc;
-  if ((rc = configure_one<4, MODE_STEP>(p, &occ))) return rc;
-  if ((rc = configure_one<4, MODE_INIT>(p, &occ))) return rc;
-  if ((rc = configure_one<4, MODE_LAST>(p, &occ))) return rc;
+  // small tiles: several CTAs per SM hide each other's bulk-copy waits and barriers
+  p->threads = (p->smem_bytes + 1024) * kTileSmallCtas <= 227u * 1024u ? kTileSmallThreads
+                                                                        : kTileThreads;
+  if (p->threads == kTileThreads) {
+    if ((rc = configure_all<kTileThreads>(p, &occ))) return rc;
+  } else {
+    if ((rc = configure_all<kTileSmallThreads>(p, &occ))) return rc;
+  }
   int dev = 0, sms = 148;
   POLFED_CUDA(cudaGetDevice(&dev));
   POLFED_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
