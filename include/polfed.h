@@ -127,7 +127,9 @@ int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_ter
  * 4 <= n_sites <= 26, no dense block,
  * off-diagonal terms of kind EXCH or HOPJW only, at most 4 distinct |amp| and 24 hops per state
  * inside a tile.  Used by polfed_filter_apply for s in {16, 32}; every other entry point uses
- * the CSR. */
+ * the CSR.  The tiled sweeps keep a tile counter inside the handle: do not run two filter
+ * applications on the same POLFED_FORMAT_TILED handle concurrently (two streams or two threads);
+ * back-to-back calls on one stream are fine. */
 
 /* Wrap a caller-owned device CSR (any real symmetric matrix, columns < n, row_ptr[n] == nnz).
  * The arrays are NOT copied and must outlive the handle. */
