@@ -248,8 +248,13 @@ def run_cuda(args):
     # (measured: config 5 4.8 vs 6.9 ms per step; config 3, tiles of <= 252 rows, 52 vs 35 us)
     tiled = args.format == "tiled" or (args.format == "auto" and w.n_up >= 0 and w.s in (16, 32)
                                        and not w.dot_bits and w.n_sites >= 24)
+    # auto: the flip format (matrix-free rows) for full-space models it supports (config 4)
+    flip = args.format == "flip" or (args.format == "auto" and w.n_up < 0 and w.s in (8, 16, 32)
+                                     and all(t[0] in ("XX", "Z", "ZZ") for t in w.terms))
+    fmt_name = "tiled" if tiled else ("flip" if flip else "csr")
     ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense,
-                                     fmt=P.FORMAT_TILED if tiled else P.FORMAT_CSR)
+                                     fmt={"tiled": P.FORMAT_TILED, "flip": P.FORMAT_FLIP,
+                                          "csr": P.FORMAT_CSR}[fmt_name])
     torch.cuda.synchronize()
     build_s = time.perf_counter() - t0
     n, nnz, s, K = ham.n, ham.nnz, w.s, args.order
@@ -347,7 +352,7 @@ def run_cuda(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOAD_NAMES[args.config], "N": n, "nnz": nnz, "s": s,
-                       "filter_order_per_step": K, "format": "tiled" if tiled else "csr",
+                       "filter_order_per_step": K, "format": fmt_name,
                        "bytes_per_fused_launch": step_bytes(n, nnz, s),
                        "l2": "inputs exceed L2 (no flush)" if step_bytes(n, nnz, s) > 4 * 126e6
                              else "working set fits L2; not flushed (the filter re-reads it by design)",
@@ -360,12 +365,13 @@ def run_cuda(args):
             "gpu_launches": args.steps * (K + 2 if tiled else K + 1),
             "clocks": clocks.summary(),
             "roofline": {"bound": "hbm",
-                         "kernel": "tiled_sweep_kernel" if tiled else "fused_step_kernel", "achieved": achieved,
+                         "kernel": {"tiled": "tiled_sweep_kernel", "flip": "flip_step_kernel",
+                                    "csr": "fused_step_kernel"}[fmt_name], "achieved": achieved,
                          "peak": peak, "peak_source": peak_src, "unit": UNIT,
                          "frac": achieved / peak, "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS,
                          "launch_ms": kernel_ms, "launches_timed": n_l,
                          "traffic": recorded_traffic(WORKLOAD_NAMES[args.config]
-                                                    + ("/tiled" if tiled else "/csr"))},
+                                                    + "/" + fmt_name)},
         }
         if world == 1 and args.eigs:
             del Vh, Wh, V
@@ -386,7 +392,11 @@ def time_to_nev(P, config: int):
     import torch
     w = workloads.make_workload(config)
     basis = P.polfed_build_basis(w.n_sites, w.n_up)
-    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense)
+    # the flip format (matrix-free rows) where the model allows it, else CSR (the tiled format
+    # only pays on tiles larger than configs 1-3 have)
+    flip = w.n_up < 0 and w.s in (8, 16, 32) and all(t[0] in ("XX", "Z", "ZZ") for t in w.terms)
+    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense,
+                                     fmt=P.FORMAT_FLIP if flip else P.FORMAT_CSR)
     V0 = torch.from_numpy(workloads.start_block(ham.n, w.s, seed=2000 + config)).cuda()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -396,7 +406,8 @@ def time_to_nev(P, config: int):
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
     hnorm = max(abs(rep["e_min"]), abs(rep["e_max"]))
-    return {"workload": WORKLOAD_NAMES[config], "nev": w.nev, "seconds": wall,
+    return {"workload": WORKLOAD_NAMES[config], "format": "flip" if flip else "csr", "nev": w.nev,
+            "seconds": wall,
             "converged": rep["status"] == 0, "K": rep["K"], "block_steps": rep["block_steps"],
             "krylov_dim": rep["krylov_dim"], "sparse_products": rep["sparse_products"],
             "max_residual_over_normH": float(resid.max()) / hnorm,
@@ -413,8 +424,9 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--order", type=int, default=64, help="filter order K per step")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--format", default="auto", choices=["auto", "csr", "tiled"],
-                    help="auto: the tiled format where the library supports it and n_sites >= 24, else CSR")
+    ap.add_argument("--format", default="auto", choices=["auto", "csr", "tiled", "flip"],
+                    help="auto: tiled where supported and n_sites >= 24, flip for full-space XX models, "
+                         "else CSR")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--eigs", default="1,2,3",
                     help="configs whose full eigen-solve is timed at N=1 ('' to skip; 4 takes minutes)")

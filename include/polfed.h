@@ -100,7 +100,8 @@ typedef struct {
 enum {
   POLFED_FORMAT_CSR = 0,
   POLFED_FORMAT_SELL = 1, /* not implemented: POLFED_EINVAL */
-  POLFED_FORMAT_TILED = 2 /* CSR plus the tiled structured format below */
+  POLFED_FORMAT_TILED = 2, /* CSR plus the tiled structured format below */
+  POLFED_FORMAT_FLIP = 3   /* CSR plus the matrix-free flip format below */
 };
 
 /* Assemble H on the device as CSR: row_ptr int32[N+1], col int32[nnz] ascending within a
@@ -130,6 +131,16 @@ int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_ter
  * the CSR.  The tiled sweeps keep a tile counter inside the handle: do not run two filter
  * applications on the same POLFED_FORMAT_TILED handle concurrently (two streams or two threads);
  * back-to-back calls on one stream are fine. */
+
+/* POLFED_FORMAT_FLIP (matrix-free rows for full-space spin models, the paper's Fig. 7 kernel
+ * `newstate = state XOR mask`; the quantum sun Eq. 67): besides the CSR, the
+ * handle keeps the diagonal, the dense block embedded in an 8 x 8 matrix on bits 0-2 and one
+ * (mask, amplitude) pair per XX term.  Every fused step on the handle with s in {8, 16, 32}
+ * (polfed_fused_step, polfed_filter_apply, the eigen-solver, KPM) then generates the rows from
+ * the masks: eight consecutive rows are held in registers, the dense part is applied there and
+ * each XX term reads the eight rows of one partner block; same result up to rounding order.
+ * Requirements (else POLFED_EINVAL): full space (n_up < 0), 3 <= n_sites <= 31, dense block on
+ * at most 3 bits, off-diagonal terms of kind XX only, at most 64 of them outside bits 0-2. */
 
 /* Wrap a caller-owned device CSR (any real symmetric matrix, columns < n, row_ptr[n] == nnz).
  * The arrays are NOT copied and must outlive the handle. */

@@ -67,6 +67,7 @@ int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const 
 int polfed_ham_destroy(polfed_ham* ham) {
   if (!ham) return POLFED_OK;
   polfed::destroy_tiled_plan(ham->tiled);
+  polfed::destroy_flip_plan(ham->flip);
   if (ham->owns) {
     cudaFree(const_cast<int32_t*>(ham->d_row_ptr));
     cudaFree(const_cast<int32_t*>(ham->d_col));

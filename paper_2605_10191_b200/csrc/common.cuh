@@ -50,6 +50,7 @@ struct DevTerm {
 };
 
 struct TiledPlan;  // tiled.cuh
+struct FlipPlan;   // flip.cuh
 
 // assemble.cu: CSR of a term list over a basis; arrays cudaMalloc'ed, owned by the caller.
 int assemble_csr(const polfed_basis* basis, const std::vector<DevTerm>& terms, int dot_bits,
@@ -64,7 +65,15 @@ size_t tiled_workspace_bytes(const polfed_ham* ham, int s);
 int tiled_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,
                        int s, const double* d_V, double* d_W, void* d_work, cudaStream_t st);
 
-// spmm_clenshaw.cu: the fused step without argument validation.
+// flip.cu: the flip (matrix-free, full-space) format, see flip.cuh.
+int build_flip_plan(const polfed_basis* basis, const std::vector<DevTerm>& terms, int dot_bits,
+                    const double* h_dot, const polfed_ham* ham, cudaStream_t st, FlipPlan** out);
+void destroy_flip_plan(FlipPlan* plan);
+bool flip_supports(const polfed_ham* ham, int s);
+int flip_step(const polfed_ham* ham, int s, double p, double q, double r, double c, const double* X,
+              const double* Z, const double* V, double* Y, cudaStream_t st);
+
+// spmm_clenshaw.cu: the fused step without argument validation (flip handles: flip_step).
 int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
                   const double* X, const double* Z, const double* V, double* Y, cudaStream_t st);
 
@@ -97,4 +106,5 @@ struct polfed_ham {
   bool owns = false;  // arrays allocated by polfed_build_hamiltonian
   int sm_count = 148;
   polfed::TiledPlan* tiled = nullptr;  // POLFED_FORMAT_TILED only (owned)
+  polfed::FlipPlan* flip = nullptr;    // POLFED_FORMAT_FLIP only (owned)
 };
