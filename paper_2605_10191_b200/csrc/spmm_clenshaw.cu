@@ -20,11 +20,14 @@ namespace {
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 
-template <int S>
+// VEC doubles per lane: 4 (256-bit accesses) for S >= 16 when every block is 32-byte aligned --
+// half the lanes per row, so half the quad shuffles per stored entry (a shuffle costs two LSU
+// cycles, a 128-byte gather one: profiles/r01_flip_config4.md) -- else 2, else 1.
+template <int S, int VEC_>
 struct Shape {
-  static constexpr int VEC = (S >= 2) ? 2 : 1;  // doubles per lane
-  static constexpr int LPR = S / VEC;           // lanes per row
-  static constexpr int RPW = 32 / LPR;          // rows per warp
+  static constexpr int VEC = VEC_;
+  static constexpr int LPR = S / VEC;   // lanes per row
+  static constexpr int RPW = 32 / LPR;  // rows per warp
 };
 
 template <int VEC>
@@ -36,7 +39,11 @@ struct Acc {
 template <int VEC>
 __device__ __forceinline__ Acc<VEC> load_gather(const double* p) {  // X rows: keep in L1/L2
   Acc<VEC> a;
-  if constexpr (VEC == 2) {
+  if constexpr (VEC == 4) {
+    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+                 : "=d"(a.v[0]), "=d"(a.v[1]), "=d"(a.v[2]), "=d"(a.v[3])
+                 : "l"(p));
+  } else if constexpr (VEC == 2) {
     double2 t = __ldg(reinterpret_cast<const double2*>(p));
     a.v[0] = t.x;
     a.v[1] = t.y;
@@ -49,7 +56,11 @@ __device__ __forceinline__ Acc<VEC> load_gather(const double* p) {  // X rows: k
 template <int VEC>
 __device__ __forceinline__ Acc<VEC> load_stream(const double* p) {  // Z, V: touched once
   Acc<VEC> a;
-  if constexpr (VEC == 2) {
+  if constexpr (VEC == 4) {
+    asm volatile("ld.global.cs.v4.f64 {%0,%1,%2,%3}, [%4];"
+                 : "=d"(a.v[0]), "=d"(a.v[1]), "=d"(a.v[2]), "=d"(a.v[3])
+                 : "l"(p));
+  } else if constexpr (VEC == 2) {
     double2 t = __ldcs(reinterpret_cast<const double2*>(p));
     a.v[0] = t.x;
     a.v[1] = t.y;
@@ -61,20 +72,24 @@ __device__ __forceinline__ Acc<VEC> load_stream(const double* p) {  // Z, V: tou
 
 template <int VEC>
 __device__ __forceinline__ void store_stream(double* p, const Acc<VEC>& a) {
-  if constexpr (VEC == 2) {
+  if constexpr (VEC == 4) {
+    asm volatile("st.global.cs.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a.v[0]), "d"(a.v[1]),
+                 "d"(a.v[2]), "d"(a.v[3])
+                 : "memory");
+  } else if constexpr (VEC == 2) {
     __stcs(reinterpret_cast<double2*>(p), make_double2(a.v[0], a.v[1]));
   } else {
     __stcs(p, a.v[0]);
   }
 }
 
-template <int S, bool USE_Z, bool USE_V>
+template <int S, int VEC_, bool USE_Z, bool USE_V>
 __global__ void __launch_bounds__(kThreads)
 fused_step_kernel(int n, const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col,
                   const double* __restrict__ val, const double* __restrict__ X, const double* Z,
                   const double* V, double* Y, double p, double q, double r, double c,
                   int rows_per_cta) {
-  using Sh = Shape<S>;
+  using Sh = Shape<S, VEC_>;
   constexpr int VEC = Sh::VEC, LPR = Sh::LPR, RPW = Sh::RPW;
   const int lane = threadIdx.x & 31;
   const int warp = threadIdx.x >> 5;
@@ -165,10 +180,10 @@ __global__ void __launch_bounds__(256) scale_copy_kernel(size_t len2, const doub
 
 __global__ void scale_copy_tail_kernel(const double* V, double* Y, double c) { Y[0] = c * V[0]; }
 
-template <int S>
-int launch_step(const polfed_ham* ham, double p, double q, double r, double c, const double* X,
-                const double* Z, const double* V, double* Y, cudaStream_t st) {
-  using Sh = Shape<S>;
+template <int S, int VEC>
+int launch_step_v(const polfed_ham* ham, double p, double q, double r, double c, const double* X,
+                  const double* Z, const double* V, double* Y, cudaStream_t st) {
+  using Sh = Shape<S, VEC>;
   const int n = (int)ham->n;
   if (n == 0) return POLFED_OK;
   const int rows_per_pass = kWarps * Sh::RPW;
@@ -179,7 +194,7 @@ int launch_step(const polfed_ham* ham, double p, double q, double r, double c, c
   const unsigned grid = (unsigned)((n + (long long)rows_per_cta - 1) / rows_per_cta);
   const bool uz = (r != 0.0), uv = (c != 0.0);
 #define POLFED_GO(UZ, UV)                                                                      \
-  fused_step_kernel<S, UZ, UV><<<grid, kThreads, 0, st>>>(n, ham->d_row_ptr, ham->d_col,       \
+  fused_step_kernel<S, VEC, UZ, UV><<<grid, kThreads, 0, st>>>(n, ham->d_row_ptr, ham->d_col,  \
                                                           ham->d_val, X, Z, V, Y, p, q, r, c,  \
                                                           rows_per_cta)
   if (uz && uv) POLFED_GO(true, true);
@@ -189,6 +204,18 @@ int launch_step(const polfed_ham* ham, double p, double q, double r, double c, c
 #undef POLFED_GO
   POLFED_LAUNCH_CHECK("fused_step_kernel");
   return POLFED_OK;
+}
+
+inline bool aligned32(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 31u) == 0; }
+
+template <int S>
+int launch_step(const polfed_ham* ham, double p, double q, double r, double c, const double* X,
+                const double* Z, const double* V, double* Y, cudaStream_t st) {
+  if constexpr (S >= 16) {
+    if (aligned32(X) && aligned32(Y) && (r == 0.0 || aligned32(Z)) && (c == 0.0 || aligned32(V)))
+      return launch_step_v<S, 4>(ham, p, q, r, c, X, Z, V, Y, st);
+  }
+  return launch_step_v<S, (S >= 2) ? 2 : 1>(ham, p, q, r, c, X, Z, V, Y, st);
 }
 
 }  // namespace
