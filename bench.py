@@ -251,10 +251,10 @@ def run_cuda(args):
     # auto: the flip format (matrix-free rows) for full-space models it supports (config 4)
     flip = args.format == "flip" or (args.format == "auto" and w.n_up < 0 and w.s in (8, 16, 32)
                                      and all(t[0] in ("XX", "Z", "ZZ") for t in w.terms))
-    fmt_name = "tiled" if tiled else ("flip" if flip else "csr")
+    fmt_name = "tiled" if tiled else ("flip" if flip else ("sell" if args.format == "sell" else "csr"))
     ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense,
                                      fmt={"tiled": P.FORMAT_TILED, "flip": P.FORMAT_FLIP,
-                                          "csr": P.FORMAT_CSR}[fmt_name])
+                                          "sell": P.FORMAT_SELL, "csr": P.FORMAT_CSR}[fmt_name])
     torch.cuda.synchronize()
     build_s = time.perf_counter() - t0
     n, nnz, s, K = ham.n, ham.nnz, w.s, args.order
@@ -366,6 +366,7 @@ def run_cuda(args):
             "clocks": clocks.summary(),
             "roofline": {"bound": "hbm",
                          "kernel": {"tiled": "tiled_sweep_kernel", "flip": "flip_step_kernel",
+                                    "sell": "sell_step_kernel",
                                     "csr": "fused_step_kernel"}[fmt_name], "achieved": achieved,
                          "peak": peak, "peak_source": peak_src, "unit": UNIT,
                          "frac": achieved / peak, "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS,
@@ -424,7 +425,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--order", type=int, default=64, help="filter order K per step")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--format", default="auto", choices=["auto", "csr", "tiled", "flip"],
+    ap.add_argument("--format", default="auto", choices=["auto", "csr", "sell", "tiled", "flip"],
                     help="auto: tiled where supported and n_sites >= 24, flip for full-space XX models, "
                          "else CSR")
     ap.add_argument("--no-cpu-baseline", action="store_true")

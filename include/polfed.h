@@ -99,7 +99,7 @@ typedef struct {
 
 enum {
   POLFED_FORMAT_CSR = 0,
-  POLFED_FORMAT_SELL = 1, /* not implemented: POLFED_EINVAL */
+  POLFED_FORMAT_SELL = 1,  /* CSR plus SELL-8-sigma, see below */
   POLFED_FORMAT_TILED = 2, /* CSR plus the tiled structured format below */
   POLFED_FORMAT_FLIP = 3   /* CSR plus the matrix-free flip format below */
 };
@@ -131,6 +131,16 @@ int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_ter
  * the CSR.  The tiled sweeps keep a tile counter inside the handle: do not run two filter
  * applications on the same POLFED_FORMAT_TILED handle concurrently (two streams or two threads);
  * back-to-back calls on one stream are fine. */
+
+/* POLFED_FORMAT_SELL (SELL-C-sigma, C = 8, sigma = 128): besides the CSR, the handle keeps the
+ * rows sorted by falling length inside windows of 128 rows, cut into slices of 8 rows stored
+ * column-major and padded to the longest row of the slice.  Every fused step on the handle with
+ * s in {8, 16, 32} (for s >= 16: blocks aligned to 32 bytes, else the CSR kernel runs) reads its
+ * entries from these slices: four lanes per row, a warp per slice, entries addressed directly
+ * instead of broadcast by shuffles.  Any term list; same result as the CSR kernel (same order of
+ * the row sum).  Costs a second copy of the matrix (12 bytes per stored entry plus padding).
+ * Measured slower than the CSR kernel on configs 3 and 5: an evaluated
+ * alternative, not the default. */
 
 /* POLFED_FORMAT_FLIP (matrix-free rows for full-space spin models, the paper's Fig. 7 kernel
  * `newstate = state XOR mask`; the quantum sun Eq. 67): besides the CSR, the

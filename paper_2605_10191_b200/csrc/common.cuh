@@ -51,6 +51,7 @@ struct DevTerm {
 
 struct TiledPlan;  // tiled.cuh
 struct FlipPlan;   // flip.cuh
+struct SellPlan;   // sell.cuh
 
 // assemble.cu: CSR of a term list over a basis; arrays cudaMalloc'ed, owned by the caller.
 int assemble_csr(const polfed_basis* basis, const std::vector<DevTerm>& terms, int dot_bits,
@@ -73,7 +74,16 @@ bool flip_supports(const polfed_ham* ham, int s);
 int flip_step(const polfed_ham* ham, int s, double p, double q, double r, double c, const double* X,
               const double* Z, const double* V, double* Y, cudaStream_t st);
 
-// spmm_clenshaw.cu: the fused step without argument validation (flip handles: flip_step).
+// sell.cu: SELL-8-sigma, see sell.cuh.
+int build_sell_plan(const polfed_ham* ham, cudaStream_t st, SellPlan** out);
+void destroy_sell_plan(SellPlan* plan);
+bool sell_supports(const polfed_ham* ham, int s, const void* X, const void* Z, const void* V,
+                   const void* Y);
+int sell_step(const polfed_ham* ham, int s, double p, double q, double r, double c, const double* X,
+              const double* Z, const double* V, double* Y, cudaStream_t st);
+
+// spmm_clenshaw.cu: the fused step without argument validation (flip handles: flip_step, SELL
+// handles: sell_step).
 int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
                   const double* X, const double* Z, const double* V, double* Y, cudaStream_t st);
 
@@ -107,4 +117,5 @@ struct polfed_ham {
   int sm_count = 148;
   polfed::TiledPlan* tiled = nullptr;  // POLFED_FORMAT_TILED only (owned)
   polfed::FlipPlan* flip = nullptr;    // POLFED_FORMAT_FLIP only (owned)
+  polfed::SellPlan* sell = nullptr;    // POLFED_FORMAT_SELL only (owned)
 };

@@ -117,7 +117,7 @@ def test_term_leaving_the_sector_is_an_error(P):
     with pytest.raises(P.PolfedError):
         P.polfed_build_hamiltonian(basis, [("Z", 6, 6, 1.0)])
     with pytest.raises(P.PolfedError):
-        P.polfed_build_hamiltonian(basis, [("Z", 0, 0, 1.0)], fmt=P.FORMAT_SELL)
+        P.polfed_build_hamiltonian(basis, [("Z", 0, 0, 1.0)], fmt=17)      # no such format
 
 
 # ---- one fused step ----------------------------------------------------------------------
