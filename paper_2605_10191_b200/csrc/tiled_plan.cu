@@ -2,6 +2,8 @@
 // records in processing order, tile table, the position maps between the two layouts and the
 // caller's row order, and the diagonal + cross-cut part of each layout.
 #include <algorithm>
+#include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -220,8 +222,173 @@ int build_records(int m, const std::vector<DevTerm>& low, TiledLayout* lay,
   return POLFED_OK;
 }
 
+// ---- fibre mode ------------------------------------------------------------------------------
+struct FibreTables {
+  std::vector<uint32_t> frec;      // fibre records of all classes (padded per sector)
+  std::vector<uint32_t> rrec;      // [2^m][2] row records by class_off[k] + position
+  std::vector<int32_t> inv_sigma;  // class_off[k] + ascending class rank -> position in class
+  std::vector<int> class_fib0, class_chunks;  // per class k
+};
+
+// JW sign (1 = negative) and applicability of a hop term on the m-bit configuration l.
+inline bool hop_applies(const DevTerm& t, uint32_t l, uint32_t* l2, uint32_t* sign) {
+  const int i = t.i, j = t.j;
+  if (((l >> i) & 1u) == ((l >> j) & 1u)) return false;
+  *l2 = l ^ (1u << i) ^ (1u << j);
+  uint32_t sg = t.amp < 0 ? 1u : 0u;
+  if (t.kind == POLFED_TERM_HOPJW) {
+    const int lo = std::min(i, j), hi = std::max(i, j);
+    const uint32_t between = ((1u << hi) - 1u) & ~((2u << lo) - 1u);
+    sg ^= (uint32_t)__builtin_popcount(l & between) & 1u;
+  }
+  *sign = sg;
+  return true;
+}
+
+// Rank of the g-bit configuration c among the configurations of equal popcount (ascending).
+inline int sector_rank(uint32_t c) { return (int)class_rank(c); }
+
+// Builds the fibre-mode tables of one layout; returns POLFED_EINVAL (with *fits = false) when a
+// limit of the record formats is exceeded, so that the caller can fall back to row records.
+int build_fibres(int m, int g, const std::vector<DevTerm>& low, TiledLayout* lay, TiledPlan* plan,
+                 const std::vector<int>& class_off, FibreTables* out, bool* fits) {
+  *fits = false;
+  lay->n_coef = 0;
+  std::vector<int> cls(low.size(), -1), where(low.size(), 0);  // 0 in-fibre, 1 fibre-level, 2 row
+  for (size_t t = 0; t < low.size(); ++t) {
+    const double mag = std::fabs(low[t].amp);
+    if (mag == 0.0) continue;
+    const int a = std::min(low[t].i, low[t].j), b = std::max(low[t].i, low[t].j);
+    where[t] = b < g ? 0 : (a >= g ? 1 : 2);
+    cls[t] = 0;
+    if (where[t] == 0) continue;  // in-fibre amplitudes go into the dense matrices as they are
+    int c = 0;
+    while (c < lay->n_coef && lay->coef[c] != mag) ++c;
+    if (c == lay->n_coef) {
+      if (c == kTileMaxCoef) return POLFED_OK;  // does not fit
+      lay->coef[lay->n_coef++] = mag;
+    }
+    cls[t] = c;
+  }
+  // sector sizes and the in-fibre matrices
+  int off = 0;
+  for (int j = 0; j <= kFibreMaxSites; ++j) {
+    plan->fibre_size[j] = j <= g ? (int)host_binom(g, j) : 0;
+    plan->dense_off[j] = off;
+    off += plan->fibre_size[j] * plan->fibre_size[j];
+  }
+  for (double& d : lay->dense) d = 0.0;
+  for (uint32_t c = 0; c < (1u << g); ++c) {
+    const int j = __builtin_popcount(c), f = plan->fibre_size[j];
+    for (size_t t = 0; t < low.size(); ++t) {
+      if (cls[t] < 0 || where[t] != 0) continue;
+      uint32_t c2, sg;
+      if (!hop_applies(low[t], c, &c2, &sg)) continue;
+      // row = c (output), column = c2 (input); the term is symmetric, amplitude |amp| with sign
+      lay->dense[plan->dense_off[j] + sector_rank(c) * f + sector_rank(c2)] +=
+          (sg ? -1.0 : 1.0) * std::fabs(low[t].amp);
+    }
+  }
+
+  const size_t n_cfg = (size_t)1 << m;
+  const uint32_t n_up_cfg = 1u << (m - g);
+  out->inv_sigma.assign(n_cfg, 0);
+  out->rrec.assign(n_cfg * 2, 0u);
+  out->frec.clear();
+  out->class_fib0.assign(m + 1, 0);
+  out->class_chunks.assign(m + 1, 0);
+
+  struct Fibre {
+    uint32_t u;
+    int j;
+    std::vector<Entry> hops;  // nbr = partner upper configuration (resolved to a position later)
+  };
+  for (int k = 0; k <= m; ++k) {
+    std::vector<Fibre> fibres;
+    for (uint32_t u = 0; u < n_up_cfg; ++u) {
+      const int j = k - __builtin_popcount(u);
+      if (j < 0 || j > g) continue;
+      Fibre fb{u, j, {}};
+      for (size_t t = 0; t < low.size(); ++t) {
+        if (cls[t] < 0 || where[t] != 1) continue;
+        uint32_t l2, sg;
+        if (!hop_applies(low[t], u << g, &l2, &sg)) continue;
+        fb.hops.push_back(Entry{l2 >> g, (uint32_t)cls[t], sg});
+      }
+      if ((int)fb.hops.size() > kFibreMaxHops) return POLFED_OK;
+      fibres.push_back(fb);
+    }
+    // large sectors first, then falling fibre degree: the chunks a CTA claims last are small
+    std::stable_sort(fibres.begin(), fibres.end(), [&](const Fibre& a, const Fibre& b) {
+      const int fa = plan->fibre_size[a.j], fbs = plan->fibre_size[b.j];
+      if (fa != fbs) return fa > fbs;
+      if (a.j != b.j) return a.j < b.j;
+      return a.hops.size() > b.hops.size();
+    });
+    // positions: fibres in this order, rows of a fibre ascending in the low configuration
+    std::vector<int> fibre_pos0(n_up_cfg, -1);
+    int32_t* inv = out->inv_sigma.data() + class_off[k];
+    int pos = 0;
+    for (const Fibre& fb : fibres) {
+      fibre_pos0[fb.u] = pos;
+      for (uint32_t c = 0; c < (1u << g); ++c) {
+        if (__builtin_popcount(c) != fb.j) continue;
+        inv[class_rank((fb.u << g) | c)] = pos++;
+      }
+    }
+    if (pos != class_off[k + 1] - class_off[k]) return fail(POLFED_ECUDA, "fibre tables: bad class");
+    // fibre records, padded so that a chunk of kFibresPerChunk fibres never mixes sectors
+    out->class_fib0[k] = (int)(out->frec.size() / kFibreRecWords);
+    auto emit = [&](const Fibre* fb) {
+      uint32_t w[kFibreRecWords] = {0, 0, 0, 0, 0, 0, 0, 0};
+      if (fb) {
+        w[0] = (uint32_t)fibre_pos0[fb->u] | ((uint32_t)fb->j << 11) |
+               ((uint32_t)fb->hops.size() << 14) | (1u << 18);
+        for (size_t e = 0; e < fb->hops.size(); ++e) {
+          const uint32_t p0 = (uint32_t)fibre_pos0[fb->hops[e].nbr];
+          uint32_t& word = w[1 + (e >> 1)];
+          if ((e & 1) == 0) word |= (p0 << 7) | fb->hops[e].cls | (fb->hops[e].sign << 30);
+          else word |= (p0 << 18) | (fb->hops[e].cls << 2) | (fb->hops[e].sign << 31);
+        }
+      }
+      out->frec.insert(out->frec.end(), w, w + kFibreRecWords);
+    };
+    size_t at = 0;
+    while (at < fibres.size()) {
+      size_t end = at;
+      while (end < fibres.size() && fibres[end].j == fibres[at].j) ++end;
+      for (size_t f = at; f < end; ++f) emit(&fibres[f]);
+      for (size_t f = end - at; f % kFibresPerChunk; ++f) emit(nullptr);
+      at = end;
+    }
+    out->class_chunks[k] =
+        (int)(out->frec.size() / kFibreRecWords - out->class_fib0[k]) / kFibresPerChunk;
+    // row records: hops between the low g sites and the rest
+    for (const Fibre& fb : fibres)
+      for (uint32_t c = 0; c < (1u << g); ++c) {
+        if (__builtin_popcount(c) != fb.j) continue;
+        const uint32_t l = (fb.u << g) | c;
+        uint32_t ent[kFibreRowHops], cnt = 0;
+        for (size_t t = 0; t < low.size(); ++t) {
+          if (cls[t] < 0 || where[t] != 2) continue;
+          uint32_t l2, sg;
+          if (!hop_applies(low[t], l, &l2, &sg)) continue;
+          if (cnt == kFibreRowHops) return POLFED_OK;
+          ent[cnt++] = (uint32_t)inv[class_rank(l2)] | ((uint32_t)cls[t] << 11) | (sg << 13);
+        }
+        uint32_t* w = out->rrec.data() + ((size_t)class_off[k] + inv[class_rank(l)]) * 2;
+        w[0] = (cnt > 0 ? ent[0] : 0u) | ((cnt > 1 ? ent[1] : 0u) << 14) | (cnt << 28);
+        w[1] = cnt > 2 ? ent[2] : 0u;
+      }
+  }
+  *fits = true;
+  return POLFED_OK;
+}
+
 void free_layout(TiledLayout& l) {
   cudaFree(l.d_records);
+  cudaFree(l.d_fibre_rec);
+  cudaFree(l.d_row_rec);
   cudaFree(l.d_diag);
   cudaFree(l.d_side);
   cudaFree(l.d_to_other);
@@ -250,6 +417,8 @@ void destroy_tiled_plan(TiledPlan* p) {
   for (auto& l : p->lay) free_layout(l);
   cudaFree(p->d_tile_row0);
   cudaFree(p->d_tile_rec0);
+  cudaFree(p->d_tile_fib0);
+  cudaFree(p->d_tile_chunks);
   cudaFree(p->d_counter);
   delete p;
 }
@@ -304,13 +473,14 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
 
   std::vector<int> class_off(m + 2, 0);
   for (int k = 0; k <= m; ++k) class_off[k + 1] = class_off[k] + (int)host_binom(m, k);
-  std::vector<int32_t> row0, rec0;
+  std::vector<int32_t> row0, rec0, tile_class;
   long long rows = 0;
   for (uint32_t h = 0; h < (1u << (L - m)); ++h) {
     const int k = n_up - __builtin_popcount(h);
     if (k < 0 || k > m) continue;
     row0.push_back((int32_t)rows);
     rec0.push_back(class_off[k]);
+    tile_class.push_back(k);
     const int nr = (int)host_binom(m, k);
     rows += nr;
     p->max_tile_rows = std::max(p->max_tile_rows, nr);
@@ -338,14 +508,48 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
                 (long long)n, kCrossPosBits);
   const unsigned row_grid = (unsigned)((n + 255) / 256);
 
+  // Fibre mode (opt-in) where the record formats allow it, else row records: g low sites per fibre.
+  FibreTables ft[2];
+  // Experimental: a third fewer shared-memory wavefronts but slower so far, so
+  // the row-record sweep stays the default; POLFED_TILED_FIBRE=1 at build time selects it.
+  int g = getenv("POLFED_TILED_FIBRE") ? std::min(kFibreMaxSites, m - 1) : 0;
+  if (g >= 1) {
+    for (int l = 0; l < 2 && g >= 1; ++l) {
+      bool fits = false;
+      rc = build_fibres(m, g, low[l], &p->lay[l], p, class_off, &ft[l], &fits);
+      if (rc) return rc;
+      if (!fits) g = 0;
+    }
+  }
+  p->fibre_g = g >= 1 ? g : 0;
+  if (p->fibre_g) {
+    std::vector<int32_t> fib0, chunks;
+    for (int k : tile_class) {
+      fib0.push_back(ft[0].class_fib0[k]);
+      chunks.push_back(ft[0].class_chunks[k]);
+    }
+    rc = upload(&p->d_tile_fib0, fib0);
+    if (rc) return rc;
+    rc = upload(&p->d_tile_chunks, chunks);
+    if (rc) return rc;
+  }
+
   for (int l = 0; l < 2; ++l) {
     TiledLayout& lay = p->lay[l];
     std::vector<uint32_t> rec;
     std::vector<int32_t> inv_sigma;
-    rc = build_records(m, low[l], &lay, &rec, &inv_sigma, class_off);
-    if (rc) return rc;
-    rc = upload(&lay.d_records, rec);
-    if (rc) return rc;
+    if (p->fibre_g) {
+      inv_sigma = ft[l].inv_sigma;
+      rc = upload(&lay.d_fibre_rec, ft[l].frec);
+      if (rc) return rc;
+      rc = upload(&lay.d_row_rec, ft[l].rrec);
+      if (rc) return rc;
+    } else {
+      rc = build_records(m, low[l], &lay, &rec, &inv_sigma, class_off);
+      if (rc) return rc;
+      rc = upload(&lay.d_records, rec);
+      if (rc) return rc;
+    }
     int32_t* d_inv = nullptr;
     POLFED_CUDA(tmp.alloc(&d_inv, inv_sigma.size()));
     POLFED_CUDA(cudaMemcpyAsync(d_inv, inv_sigma.data(), sizeof(int32_t) * inv_sigma.size(),

@@ -45,6 +45,14 @@ struct SweepArgs {
   double pf;              // finishing scalar p_k
   double ps, qs, rs, cs;  // starting scalars of step k-1
   int mode;
+  // fibre mode (tiled.cuh)
+  const uint32_t* fibre_rec;
+  const uint32_t* row_rec;
+  const int32_t* tile_fib0;
+  const int32_t* tile_chunks;
+  int fibre_size[kFibreMaxSites + 1];
+  int dense_off[kFibreMaxSites + 1];
+  double dense[kFibreDense];
 #ifdef POLFED_TILED_PROFILE
   int skip;                  // POLFED_TILED_SKIP: parts of the sweep left out (timing only)
   unsigned long long* prof;  // per CTA: cycles in tile load / phase 2 / reload / phase 3, count
@@ -545,6 +553,343 @@ __global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSm
   }
 }
 
+// ---- fibre mode (tiled.cuh): 8 lanes own a fibre of up to 10 rows ----------------------------
+
+__device__ __forceinline__ int grab_one(int* counter, int lane) {  // a warp claims one chunk
+  int v = 0;
+  if (lane == 0) v = atomicAdd(counter, 1);
+  return __shfl_sync(0xffffffffu, v, 0);
+}
+
+__device__ __forceinline__ double2 ldg128(const double* p) {
+  return __ldg(reinterpret_cast<const double2*>(p));
+}
+__device__ __forceinline__ double2 ldg128_stream(const double* p, uint64_t pol) {
+  double2 r;
+  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;"
+               : "=d"(r.x), "=d"(r.y)
+               : "l"(p), "l"(pol));
+  return r;
+}
+__device__ __forceinline__ void stg128_hint(double* p, const double2 r, uint64_t pol) {
+  asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p),
+               "d"(r.x), "d"(r.y), "l"(pol)
+               : "memory");
+}
+__device__ __forceinline__ void fma2(double c, const double2 x, double2& acc) {
+  acc.x = fma(c, x.x, acc.x);
+  acc.y = fma(c, x.y, acc.y);
+}
+
+// The per-row records of a fibre (contiguous rows) are read row by row after the hops; ask for
+// their lines at the start of the chunk so that those reads hit L1.
+__device__ __forceinline__ void prefetch_l1(const void* p) {
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+}
+__device__ __forceinline__ void fibre_prefetch(const void* base, int first, int count, int elem_bytes,
+                                               int l8) {
+  if (count <= 0) return;
+  const char* p0 = static_cast<const char*>(base) + (size_t)first * elem_bytes;
+  const char* p1 = p0 + (size_t)count * elem_bytes - 1;
+  const char* line = reinterpret_cast<const char*>((reinterpret_cast<uintptr_t>(p0) & ~(uintptr_t)127)) +
+                     128 * l8;
+  if (line <= p1) prefetch_l1(line);
+}
+
+// Header of a fibre record.
+struct FibreHead {
+  int pos0, rows, n_hops, dense_off;
+};
+__device__ __forceinline__ FibreHead fibre_head(uint32_t h, const SweepArgs& a) {
+  FibreHead f;
+  const int j = (h >> 11) & 7;
+  f.pos0 = h & 0x7ff;
+  f.n_hops = (h >> 14) & 15;
+  f.rows = ((h >> 18) & 1u) ? a.fibre_size[j] : 0;
+  f.dense_off = a.dense_off[j];
+  return f;
+}
+
+// acc[r] += (in-fibre hops + `self` x own row) for the rows of the fibre held in xo.
+__device__ __forceinline__ void fibre_dense(const SweepArgs& a, const FibreHead& f,
+                                            const double2 (&xo)[kFibreMaxRows],
+                                            double2 (&acc)[kFibreMaxRows]) {
+#pragma unroll
+  for (int r = 0; r < kFibreMaxRows; ++r) {
+    if (r >= f.rows) break;
+    const double* m = a.dense + f.dense_off + r * f.rows;
+#pragma unroll
+    for (int c = 0; c < kFibreMaxRows; ++c) {
+      if (c >= f.rows) break;
+      fma2(m[c], xo[c], acc[r]);
+    }
+  }
+}
+
+// Hops among the upper tile sites: one entry moves the whole fibre.  w_me is this lane's word of
+// the fibre record (lane l8 holds word l8); max_hops is warp-uniform.
+template <int NC>
+__device__ __forceinline__ void fibre_hops(const SweepArgs& a, const FibreHead& f, uint32_t w_me,
+                                           int max_hops, const unsigned char* __restrict__ xl,
+                                           double2 (&acc)[kFibreMaxRows]) {
+#pragma unroll
+  for (int w = 1; w < kFibreRecWords; ++w) {
+    if (2 * (w - 1) >= max_hops) break;
+    const uint32_t word = __shfl_sync(0xffffffffu, w_me, w, 8);
+    if (2 * (w - 1) < f.n_hops) {
+      const double cf = signed_coef(pick_coef<NC>(word & 3u, a.coef), word << 1);
+      const unsigned char* src = xl + (word & 0x3ff80u);
+#pragma unroll
+      for (int r = 0; r < kFibreMaxRows; ++r) {
+        if (r >= f.rows) break;
+        fma2(cf, *reinterpret_cast<const double2*>(src + r * 128), acc[r]);
+      }
+    }
+    if (2 * w - 1 < f.n_hops) {
+      const double cf = signed_coef(pick_coef<NC>((word >> 2) & 3u, a.coef), word);
+      const unsigned char* src = xl + ((word >> 11) & 0x3ff80u);
+#pragma unroll
+      for (int r = 0; r < kFibreMaxRows; ++r) {
+        if (r >= f.rows) break;
+        fma2(cf, *reinterpret_cast<const double2*>(src + r * 128), acc[r]);
+      }
+    }
+  }
+}
+
+// Hops between the low g sites and the rest: up to three neighbours of one row (row record rr).
+template <int NC>
+__device__ __forceinline__ void row_hops(const SweepArgs& a, const uint2 rr,
+                                         const unsigned char* __restrict__ xl, double2& acc) {
+  const uint32_t cnt = rr.x >> 28;
+  const uint32_t e[kFibreRowHops] = {rr.x & 0x3fffu, (rr.x >> 14) & 0x3fffu, rr.y & 0x3fffu};
+#pragma unroll
+  for (int i = 0; i < kFibreRowHops; ++i)
+    if ((uint32_t)i < cnt) {
+      const double cf = signed_coef(pick_coef<NC>((e[i] >> 11) & 3u, a.coef), e[i] << 18);
+      fma2(cf, *reinterpret_cast<const double2*>(xl + (e[i] & 0x7ffu) * 128u), acc);
+    }
+}
+
+template <int NC, int MODE, int THREADS>
+__global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSmallCtas)
+    tiled_fibre_kernel(const SweepArgs a) {
+  constexpr int kIterRows = (THREADS / 32) * kRowsPerIter;  // MODE_INIT's static loop
+  extern __shared__ __align__(128) unsigned char smem_raw[];  // the tile panel
+  __shared__ uint64_t bar;
+  __shared__ int s_tile[2];
+  __shared__ int s_chunk[2];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int grp = lane >> 3, l8 = lane & 7;       // fibre of the chunk, 16-byte slice of a row
+  const unsigned char* xl = smem_raw + 16 * l8;
+  if (tid == 0) {
+    mbar_init(&bar, 1);
+    s_tile[0] = atomicAdd(a.counter, 1);
+    s_chunk[0] = s_chunk[1] = 0;
+  }
+  __syncthreads();
+  unsigned parity = 0;
+  int phase = 0;
+  double* scratch = a.scratch + (size_t)blockIdx.x * a.max_tile_rows * kTilePanel;
+  const size_t panel_stride = (size_t)a.n * kTilePanel;
+  const uint64_t pol_first = l2_policy_evict_first(), pol_last = l2_policy_evict_last();
+  const double2 zero2 = make_double2(0.0, 0.0);
+
+  for (int it = 0;; ++it) {
+    const int tile = s_tile[it & 1];
+    if (tile >= a.n_tiles) break;
+    if (tid == 0) s_tile[(it + 1) & 1] = atomicAdd(a.counter, 1);
+    const int row0 = __ldg(a.tile_row0 + tile);
+    const int nrows = __ldg(a.tile_row0 + tile + 1) - row0;
+    const int n_chunks = __ldg(a.tile_chunks + tile);
+    const uint32_t* frec = a.fibre_rec + (size_t)__ldg(a.tile_fib0 + tile) * kFibreRecWords;
+    const uint2* rrec = reinterpret_cast<const uint2*>(a.row_rec) + __ldg(a.tile_rec0 + tile);
+    const uint32_t* side = a.side + (size_t)row0 * a.side_words;
+    const double* diag = a.diag + row0;
+    const int32_t* dst_map = a.dst_map + row0;
+    __syncthreads();
+
+    for (int panel = 0; panel < a.n_panels; ++panel) {
+      const double* X1 = a.X1 + panel * panel_stride;
+      const double* Pk = a.Pk + panel * panel_stride + (size_t)row0 * kTilePanel;
+      const double* V = a.V + panel * panel_stride + (size_t)row0 * kTilePanel;
+      double* Bout = a.Bout + panel * panel_stride;
+      double* Pout = a.Pout + panel * panel_stride;
+
+      if (MODE == MODE_INIT) {
+        // ---- b_K = c_K V: four lanes per row, 32 bytes each ---------------------------------
+        const int q = lane & 3;
+        for (int pos = warp * kRowsPerIter + (lane >> 2); pos < nrows; pos += kIterRows) {
+          const int dst = __ldg(dst_map + pos);
+          D4 b = ldg256_stream(V + (size_t)pos * kTilePanel + 4 * q, pol_first);
+          b.x *= a.cK;
+          b.y *= a.cK;
+          b.z *= a.cK;
+          b.w *= a.cK;
+          stg256_hint(Bout + (size_t)dst * kTilePanel + 4 * q, b, pol_first);
+          stg256_hint(scratch + (size_t)pos * kTilePanel + 4 * q, b, pol_last);
+        }
+      } else {
+        // ---- phase 2: b_k = P_k + p_k (O_l + DM) b_{k+1} ---------------------------------------
+        if (tid == 0) {
+          tile_load(smem_raw, X1 + (size_t)row0 * kTilePanel, (unsigned)nrows * 128u, &bar,
+                    pol_last);
+          s_chunk[(phase + 1) & 1] = 0;
+        }
+        int* const chunk = &s_chunk[phase & 1];
+        ++phase;
+        int c = grab_one(chunk, lane), c_n = grab_one(chunk, lane);
+        uint32_t w_n = c < n_chunks
+                           ? __ldg(frec + (size_t)(c * kFibresPerChunk + grp) * kFibreRecWords + l8)
+                           : 0u;
+        mbar_wait(&bar, parity);
+        parity ^= 1u;
+        for (; c < n_chunks; c = c_n, c_n = grab_one(chunk, lane)) {
+          const uint32_t w_me = w_n;
+          w_n = c_n < n_chunks
+                    ? __ldg(frec + (size_t)(c_n * kFibresPerChunk + grp) * kFibreRecWords + l8)
+                    : 0u;
+          const FibreHead f = fibre_head(__shfl_sync(0xffffffffu, w_me, 0, 8), a);
+          const int max_hops = __reduce_max_sync(0xffffffffu, f.n_hops);
+          fibre_prefetch(side, f.pos0, f.rows, 4 * a.side_words, l8);
+          fibre_prefetch(rrec, f.pos0, f.rows, 8, l8);
+          if (MODE == MODE_LAST) fibre_prefetch(dst_map, f.pos0, f.rows, 4, l8);
+          double2 xo[kFibreMaxRows], acc[kFibreMaxRows];
+#pragma unroll
+          for (int r = 0; r < kFibreMaxRows; ++r) {
+            xo[r] = zero2;
+            acc[r] = zero2;
+            if (r < f.rows) {
+              xo[r] = *reinterpret_cast<const double2*>(xl + (size_t)(f.pos0 + r) * 128);
+              const double dg = __ldg(diag + f.pos0 + r);
+              acc[r].x = dg * xo[r].x;
+              acc[r].y = dg * xo[r].y;
+            }
+          }
+          fibre_dense(a, f, xo, acc);
+          // the rows' share of P_k replaces the own rows in the registers and flies during the hops
+#pragma unroll
+          for (int r = 0; r < kFibreMaxRows; ++r)
+            if (r < f.rows)
+              xo[r] = ldg128_stream(Pk + (size_t)(f.pos0 + r) * kTilePanel + 2 * l8, pol_first);
+          fibre_hops<NC>(a, f, w_me, max_hops, xl, acc);
+#pragma unroll
+          for (int r = 0; r < kFibreMaxRows; ++r) {
+            if (r >= f.rows) break;
+            const int pos = f.pos0 + r;
+            const uint2 rr = __ldg(rrec + pos);
+            const uint4 sd = __ldg(reinterpret_cast<const uint4*>(side + (size_t)pos * a.side_words));
+            double2 g0 = zero2, g1 = zero2, g2 = zero2;
+            if (sd.y != kCrossNone)
+              g0 = ldg128(X1 + (size_t)(sd.y & kCrossPosMask) * kTilePanel + 2 * l8);
+            if (sd.z != kCrossNone)
+              g1 = ldg128(X1 + (size_t)(sd.z & kCrossPosMask) * kTilePanel + 2 * l8);
+            if (sd.w != kCrossNone)
+              g2 = ldg128(X1 + (size_t)(sd.w & kCrossPosMask) * kTilePanel + 2 * l8);
+            row_hops<NC>(a, rr, xl, acc[r]);
+            fma2(signed_coef(a.ccoef[(sd.y >> kCrossPosBits) & 15u], sd.y), g0, acc[r]);
+            fma2(signed_coef(a.ccoef[(sd.z >> kCrossPosBits) & 15u], sd.z), g1, acc[r]);
+            fma2(signed_coef(a.ccoef[(sd.w >> kCrossPosBits) & 15u], sd.w), g2, acc[r]);
+            if (a.side_words > 4) {  // cross-cut words 3..6 (wide cuts only)
+              const uint4 more =
+                  __ldg(reinterpret_cast<const uint4*>(side + (size_t)pos * 8 + 4));
+              const uint32_t cw[4] = {more.x, more.y, more.z, more.w};
+#pragma unroll
+              for (int j = 0; j < 4; ++j)
+                if (cw[j] != kCrossNone)
+                  fma2(signed_coef(a.ccoef[(cw[j] >> kCrossPosBits) & 15u], cw[j]),
+                       ldg128(X1 + (size_t)(cw[j] & kCrossPosMask) * kTilePanel + 2 * l8), acc[r]);
+            }
+            double2 b;
+            b.x = fma(a.pf, acc[r].x, xo[r].x);
+            b.y = fma(a.pf, acc[r].y, xo[r].y);
+            if (MODE == MODE_LAST) {
+              const int dst = __ldg(dst_map + pos);
+              stg128_hint(a.W + (size_t)dst * a.w_ld + panel * kTilePanel + 2 * l8, b, pol_first);
+            } else {
+              stg128_hint(Bout + (size_t)sd.x * kTilePanel + 2 * l8, b, pol_first);
+              stg128_hint(scratch + (size_t)pos * kTilePanel + 2 * l8, b, pol_last);
+            }
+          }
+        }
+      }
+      if (MODE == MODE_LAST) {
+        __syncthreads();  // the next bulk copy overwrites the tile
+        continue;
+      }
+
+      // ---- b_k becomes the shared tile ------------------------------------------------------
+      __threadfence_block();
+      fence_proxy_async();
+      __syncthreads();
+      if (tid == 0) {
+        tile_load(smem_raw, scratch, (unsigned)nrows * 128u, &bar, pol_last);
+        s_chunk[(phase + 1) & 1] = 0;
+      }
+      int* const chunk = &s_chunk[phase & 1];
+      ++phase;
+      int c = grab_one(chunk, lane), c_n = grab_one(chunk, lane);
+      uint32_t w_n = c < n_chunks
+                         ? __ldg(frec + (size_t)(c * kFibresPerChunk + grp) * kFibreRecWords + l8)
+                         : 0u;
+      if (MODE == MODE_STEP)
+        next_tile_prefetch(a, tile, s_tile[(it + 1) & 1], panel, panel_stride, tid);
+      mbar_wait(&bar, parity);
+      parity ^= 1u;
+      // the parked copy is dead once it is back in shared memory: drop it from L2 unwritten
+      for (int r = tid; r < nrows; r += THREADS)
+        asm volatile("discard.global.L2 [%0], 128;" ::"l"(scratch + (size_t)r * kTilePanel) : "memory");
+
+      // ---- phase 3: P_{k-1} = c_{k-1} V + p_{k-1} O_l b_k + q_{k-1} b_k + r b_{k+1} ------------
+      const double q_over_p = a.qs / a.ps;
+      for (; c < n_chunks; c = c_n, c_n = grab_one(chunk, lane)) {
+        const uint32_t w_me = w_n;
+        w_n = c_n < n_chunks
+                  ? __ldg(frec + (size_t)(c_n * kFibresPerChunk + grp) * kFibreRecWords + l8)
+                  : 0u;
+        const FibreHead f = fibre_head(__shfl_sync(0xffffffffu, w_me, 0, 8), a);
+        const int max_hops = __reduce_max_sync(0xffffffffu, f.n_hops);
+        fibre_prefetch(rrec, f.pos0, f.rows, 8, l8);
+        fibre_prefetch(dst_map, f.pos0, f.rows, 4, l8);
+        double2 xo[kFibreMaxRows], acc[kFibreMaxRows];
+#pragma unroll
+        for (int r = 0; r < kFibreMaxRows; ++r) {
+          xo[r] = zero2;
+          acc[r] = zero2;
+          if (r < f.rows) {
+            xo[r] = *reinterpret_cast<const double2*>(xl + (size_t)(f.pos0 + r) * 128);
+            acc[r].x = q_over_p * xo[r].x;  // q b_k, scaled by p with the hops below
+            acc[r].y = q_over_p * xo[r].y;
+          }
+        }
+        fibre_dense(a, f, xo, acc);
+#pragma unroll
+        for (int r = 0; r < kFibreMaxRows; ++r) {  // c V of the rows flies during the hops
+          xo[r] = zero2;
+          if (r < f.rows && a.cs != 0.0)
+            xo[r] = ldg128_stream(V + (size_t)(f.pos0 + r) * kTilePanel + 2 * l8, pol_first);
+        }
+        fibre_hops<NC>(a, f, w_me, max_hops, xl, acc);
+#pragma unroll
+        for (int r = 0; r < kFibreMaxRows; ++r) {
+          if (r >= f.rows) break;
+          const int pos = f.pos0 + r;
+          const uint2 rr = __ldg(rrec + pos);
+          const int dst = __ldg(dst_map + pos);
+          double2 x1 = zero2;
+          if (a.rs != 0.0) x1 = ldg128(X1 + ((size_t)row0 + pos) * kTilePanel + 2 * l8);
+          row_hops<NC>(a, rr, xl, acc[r]);
+          double2 y;
+          y.x = fma(a.cs, xo[r].x, fma(a.rs, x1.x, a.ps * acc[r].x));
+          y.y = fma(a.cs, xo[r].y, fma(a.rs, x1.y, a.ps * acc[r].y));
+          stg128_hint(Pout + (size_t)dst * kTilePanel + 2 * l8, y, pol_first);
+        }
+      }
+      __syncthreads();  // all reads of the tile done before the next bulk copy
+    }
+  }
+}
+
 // V (row-major n x s, caller's row order) -> panel-major copies at the positions of both layouts.
 __global__ void __launch_bounds__(256) tiled_pack_kernel(long long n, int n_panels,
                                                          const double* __restrict__ V,
@@ -575,8 +920,21 @@ int launch_sweep_t(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
   return POLFED_OK;
 }
 
+template <int NC, int THREADS>
+int launch_fibre_t(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
+  if (a.mode == MODE_INIT)
+    tiled_fibre_kernel<NC, MODE_INIT, THREADS><<<p->grid, THREADS, p->smem_bytes, st>>>(a);
+  else if (a.mode == MODE_LAST)
+    tiled_fibre_kernel<NC, MODE_LAST, THREADS><<<p->grid, THREADS, p->smem_bytes, st>>>(a);
+  else
+    tiled_fibre_kernel<NC, MODE_STEP, THREADS><<<p->grid, THREADS, p->smem_bytes, st>>>(a);
+  POLFED_LAUNCH_CHECK("tiled_fibre_kernel");
+  return POLFED_OK;
+}
+
 template <int NC>
 int launch_sweep(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
+  if (p->fibre_g) return launch_fibre_t<NC, kTileThreads>(p, a, st);
   return p->threads == kTileThreads ? launch_sweep_t<NC, kTileThreads>(p, a, st)
                                     : launch_sweep_t<NC, kTileSmallThreads>(p, a, st);
 }
@@ -590,6 +948,17 @@ int sweep(const TiledPlan* p, int layout, SweepArgs a, cudaStream_t st) {
   for (int c = 0; c <= kTileMaxCrossCoef; ++c) a.ccoef[c] = L.ccoef[c];
   a.dst_map = (a.mode == MODE_LAST) ? L.d_to_natural : L.d_to_other;
   for (int c = 0; c < kTileMaxCoef; ++c) a.coef[c] = L.coef[c];
+  if (p->fibre_g) {
+    a.fibre_rec = L.d_fibre_rec;
+    a.row_rec = L.d_row_rec;
+    a.tile_fib0 = p->d_tile_fib0;
+    a.tile_chunks = p->d_tile_chunks;
+    for (int j = 0; j <= kFibreMaxSites; ++j) {
+      a.fibre_size[j] = p->fibre_size[j];
+      a.dense_off[j] = p->dense_off[j];
+    }
+    for (int i = 0; i < kFibreDense; ++i) a.dense[i] = L.dense[i];
+  }
   POLFED_CUDA(cudaMemsetAsync(p->d_counter, 0, sizeof(int), st));
   return L.n_coef <= 2 ? launch_sweep<2>(p, a, st) : launch_sweep<4>(p, a, st);
 }
@@ -619,6 +988,31 @@ int configure_all(TiledPlan* p, int* occ) {
   return POLFED_OK;
 }
 
+template <int NC, int MODE, int THREADS>
+int configure_fibre_one(TiledPlan* p, int* occ) {
+  POLFED_CUDA(cudaFuncSetAttribute(tiled_fibre_kernel<NC, MODE, THREADS>,
+                                   cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)p->smem_bytes));
+  int o = 0;
+  POLFED_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+      &o, tiled_fibre_kernel<NC, MODE, THREADS>, THREADS, p->smem_bytes));
+  if (o < 1) return fail(POLFED_ECUDA, "tiled format: fibre kernel does not fit an SM");
+  *occ = (*occ == 0 || o < *occ) ? o : *occ;
+  return POLFED_OK;
+}
+
+template <int THREADS>
+int configure_fibre_all(TiledPlan* p, int* occ) {
+  int rc;
+  if ((rc = configure_fibre_one<2, MODE_STEP, THREADS>(p, occ))) return rc;
+  if ((rc = configure_fibre_one<2, MODE_INIT, THREADS>(p, occ))) return rc;
+  if ((rc = configure_fibre_one<2, MODE_LAST, THREADS>(p, occ))) return rc;
+  if ((rc = configure_fibre_one<4, MODE_STEP, THREADS>(p, occ))) return rc;
+  if ((rc = configure_fibre_one<4, MODE_INIT, THREADS>(p, occ))) return rc;
+  if ((rc = configure_fibre_one<4, MODE_LAST, THREADS>(p, occ))) return rc;
+  return POLFED_OK;
+}
+
 }  // namespace
 
 int tiled_configure_launch(TiledPlan* p) {
@@ -627,7 +1021,10 @@ int tiled_configure_launch(TiledPlan* p) {
   // small tiles: several CTAs per SM hide each other's bulk-copy waits and barriers
   p->threads = (p->smem_bytes + 1024) * kTileSmallCtas <= 227u * 1024u ? kTileSmallThreads
                                                                         : kTileThreads;
-  if (p->threads == kTileThreads) {
+  if (p->fibre_g) p->threads = kTileThreads;  // the fibre kernel needs the registers of one CTA per SM
+  if (p->fibre_g) {
+    if ((rc = configure_fibre_all<kTileThreads>(p, &occ))) return rc;
+  } else if (p->threads == kTileThreads) {
     if ((rc = configure_all<kTileThreads>(p, &occ))) return rc;
   } else {
     if ((rc = configure_all<kTileSmallThreads>(p, &occ))) return rc;
