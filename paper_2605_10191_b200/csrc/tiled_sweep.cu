@@ -10,6 +10,7 @@
 // alternate the order of the two (even row slots low chunk first, odd slots high chunk first),
 // so that the two rows of a quarter-warp always hit disjoint banks whatever rows they gather.
 #include <cstdlib>
+#include <type_traits>
 
 #include "tiled.cuh"
 
@@ -596,6 +597,14 @@ __device__ __forceinline__ void fibre_prefetch(const void* base, int first, int 
   if (line <= p1) prefetch_l1(line);
 }
 
+// Per-row records of a fibre are loaded once per chunk, one row per lane (lane l8 holds rows l8
+// and l8 + 8), before the hops, and handed to the 8 lanes row by row with shuffles: no dependent
+// global load is left in the per-row tail.  R is a compile-time row number.
+template <int R>
+__device__ __forceinline__ uint32_t row_bcast(uint32_t a_word, uint32_t b_word) {
+  return __shfl_sync(0xffffffffu, R < 8 ? a_word : b_word, R & 7, 8);
+}
+
 // Header of a fibre record.
 struct FibreHead {
   int pos0, rows, n_hops, dense_off;
@@ -751,9 +760,22 @@ __global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSm
                     : 0u;
           const FibreHead f = fibre_head(__shfl_sync(0xffffffffu, w_me, 0, 8), a);
           const int max_hops = __reduce_max_sync(0xffffffffu, f.n_hops);
-          fibre_prefetch(side, f.pos0, f.rows, 4 * a.side_words, l8);
-          fibre_prefetch(rrec, f.pos0, f.rows, 8, l8);
-          if (MODE == MODE_LAST) fibre_prefetch(dst_map, f.pos0, f.rows, 4, l8);
+          const int max_rows = __reduce_max_sync(0xffffffffu, f.rows);
+          // per-row records, one row per lane
+          uint2 rrA = make_uint2(0u, 0u), rrB = rrA;
+          uint4 sdA = make_uint4(0u, kCrossNone, kCrossNone, kCrossNone), sdB = sdA;
+          uint32_t dnA = 0u, dnB = 0u;  // MODE_LAST: row in the caller's order
+          if (l8 < f.rows) {
+            rrA = __ldg(rrec + f.pos0 + l8);
+            sdA = __ldg(reinterpret_cast<const uint4*>(side + (size_t)(f.pos0 + l8) * a.side_words));
+            if (MODE == MODE_LAST) dnA = (uint32_t)__ldg(dst_map + f.pos0 + l8);
+          }
+          if (l8 + 8 < f.rows) {
+            rrB = __ldg(rrec + f.pos0 + l8 + 8);
+            sdB = __ldg(
+                reinterpret_cast<const uint4*>(side + (size_t)(f.pos0 + l8 + 8) * a.side_words));
+            if (MODE == MODE_LAST) dnB = (uint32_t)__ldg(dst_map + f.pos0 + l8 + 8);
+          }
           double2 xo[kFibreMaxRows], acc[kFibreMaxRows];
 #pragma unroll
           for (int r = 0; r < kFibreMaxRows; ++r) {
@@ -773,23 +795,42 @@ __global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSm
             if (r < f.rows)
               xo[r] = ldg128_stream(Pk + (size_t)(f.pos0 + r) * kTilePanel + 2 * l8, pol_first);
           fibre_hops<NC>(a, f, w_me, max_hops, xl, acc);
+          {  // b_k = P_k + p (...) = p (acc + P_k / p): P_k leaves the registers before the tail
+            const double inv_pf = 1.0 / a.pf;
 #pragma unroll
-          for (int r = 0; r < kFibreMaxRows; ++r) {
-            if (r >= f.rows) break;
+            for (int r = 0; r < kFibreMaxRows; ++r) fma2(inv_pf, xo[r], acc[r]);
+          }
+          // per-row tail, two rows in flight: records of row r + 1 are handed out and its cross-cut
+          // rows requested while row r is finished
+          uint4 sd_c;
+          uint2 rr_c;
+          uint32_t dn_c = 0u;
+          double2 g_c[3];
+          auto fetch = [&](auto R, uint4& sd, uint2& rr, uint32_t& dn, double2 (&g)[3]) {
+            constexpr int RR = decltype(R)::value;
+            sd.x = row_bcast<RR>(sdA.x, sdB.x);
+            sd.y = row_bcast<RR>(sdA.y, sdB.y);
+            sd.z = row_bcast<RR>(sdA.z, sdB.z);
+            sd.w = row_bcast<RR>(sdA.w, sdB.w);
+            rr.x = row_bcast<RR>(rrA.x, rrB.x);
+            rr.y = row_bcast<RR>(rrA.y, rrB.y);
+            if (MODE == MODE_LAST) dn = row_bcast<RR>(dnA, dnB);
+            const uint32_t cw[3] = {sd.y, sd.z, sd.w};
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+              g[j] = zero2;
+              if (cw[j] != kCrossNone)
+                g[j] = ldg128(X1 + (size_t)(cw[j] & kCrossPosMask) * kTilePanel + 2 * l8);
+            }
+          };
+          auto finish = [&](int r, const uint4& sd, const uint2& rr, uint32_t dn,
+                            const double2 (&g)[3], double2& ac) {
+            if (r >= f.rows) return;
             const int pos = f.pos0 + r;
-            const uint2 rr = __ldg(rrec + pos);
-            const uint4 sd = __ldg(reinterpret_cast<const uint4*>(side + (size_t)pos * a.side_words));
-            double2 g0 = zero2, g1 = zero2, g2 = zero2;
-            if (sd.y != kCrossNone)
-              g0 = ldg128(X1 + (size_t)(sd.y & kCrossPosMask) * kTilePanel + 2 * l8);
-            if (sd.z != kCrossNone)
-              g1 = ldg128(X1 + (size_t)(sd.z & kCrossPosMask) * kTilePanel + 2 * l8);
-            if (sd.w != kCrossNone)
-              g2 = ldg128(X1 + (size_t)(sd.w & kCrossPosMask) * kTilePanel + 2 * l8);
-            row_hops<NC>(a, rr, xl, acc[r]);
-            fma2(signed_coef(a.ccoef[(sd.y >> kCrossPosBits) & 15u], sd.y), g0, acc[r]);
-            fma2(signed_coef(a.ccoef[(sd.z >> kCrossPosBits) & 15u], sd.z), g1, acc[r]);
-            fma2(signed_coef(a.ccoef[(sd.w >> kCrossPosBits) & 15u], sd.w), g2, acc[r]);
+            row_hops<NC>(a, rr, xl, ac);
+            fma2(signed_coef(a.ccoef[(sd.y >> kCrossPosBits) & 15u], sd.y), g[0], ac);
+            fma2(signed_coef(a.ccoef[(sd.z >> kCrossPosBits) & 15u], sd.z), g[1], ac);
+            fma2(signed_coef(a.ccoef[(sd.w >> kCrossPosBits) & 15u], sd.w), g[2], ac);
             if (a.side_words > 4) {  // cross-cut words 3..6 (wide cuts only)
               const uint4 more =
                   __ldg(reinterpret_cast<const uint4*>(side + (size_t)pos * 8 + 4));
@@ -798,19 +839,47 @@ __global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSm
               for (int j = 0; j < 4; ++j)
                 if (cw[j] != kCrossNone)
                   fma2(signed_coef(a.ccoef[(cw[j] >> kCrossPosBits) & 15u], cw[j]),
-                       ldg128(X1 + (size_t)(cw[j] & kCrossPosMask) * kTilePanel + 2 * l8), acc[r]);
+                       ldg128(X1 + (size_t)(cw[j] & kCrossPosMask) * kTilePanel + 2 * l8), ac);
             }
             double2 b;
-            b.x = fma(a.pf, acc[r].x, xo[r].x);
-            b.y = fma(a.pf, acc[r].y, xo[r].y);
+            b.x = a.pf * ac.x;
+            b.y = a.pf * ac.y;
             if (MODE == MODE_LAST) {
-              const int dst = __ldg(dst_map + pos);
-              stg128_hint(a.W + (size_t)dst * a.w_ld + panel * kTilePanel + 2 * l8, b, pol_first);
+              stg128_hint(a.W + (size_t)dn * a.w_ld + panel * kTilePanel + 2 * l8, b, pol_first);
             } else {
               stg128_hint(Bout + (size_t)sd.x * kTilePanel + 2 * l8, b, pol_first);
               stg128_hint(scratch + (size_t)pos * kTilePanel + 2 * l8, b, pol_last);
             }
-          }
+          };
+          fetch(std::integral_constant<int, 0>{}, sd_c, rr_c, dn_c, g_c);
+#define POLFED_FIBRE_ROW(R)                                                              \
+  if (R < max_rows) {                                                                    \
+    uint4 sd_n = make_uint4(0u, kCrossNone, kCrossNone, kCrossNone);                     \
+    uint2 rr_n = make_uint2(0u, 0u);                                                     \
+    uint32_t dn_n = 0u;                                                                  \
+    double2 g_n[3] = {zero2, zero2, zero2};                                              \
+    if (R + 1 < max_rows)                                                                \
+      fetch(std::integral_constant<int, (R + 1 < kFibreMaxRows ? R + 1 : 0)>{}, sd_n, rr_n, dn_n, \
+            g_n);                                                                        \
+    finish(R, sd_c, rr_c, dn_c, g_c, acc[R]);                                            \
+    sd_c = sd_n;                                                                         \
+    rr_c = rr_n;                                                                         \
+    dn_c = dn_n;                                                                         \
+    g_c[0] = g_n[0];                                                                     \
+    g_c[1] = g_n[1];                                                                     \
+    g_c[2] = g_n[2];                                                                     \
+  }
+          POLFED_FIBRE_ROW(0)
+          POLFED_FIBRE_ROW(1)
+          POLFED_FIBRE_ROW(2)
+          POLFED_FIBRE_ROW(3)
+          POLFED_FIBRE_ROW(4)
+          POLFED_FIBRE_ROW(5)
+          POLFED_FIBRE_ROW(6)
+          POLFED_FIBRE_ROW(7)
+          POLFED_FIBRE_ROW(8)
+          POLFED_FIBRE_ROW(9)
+#undef POLFED_FIBRE_ROW
         }
       }
       if (MODE == MODE_LAST) {
@@ -849,8 +918,17 @@ __global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSm
                   : 0u;
         const FibreHead f = fibre_head(__shfl_sync(0xffffffffu, w_me, 0, 8), a);
         const int max_hops = __reduce_max_sync(0xffffffffu, f.n_hops);
-        fibre_prefetch(rrec, f.pos0, f.rows, 8, l8);
-        fibre_prefetch(dst_map, f.pos0, f.rows, 4, l8);
+        const int max_rows = __reduce_max_sync(0xffffffffu, f.rows);
+        uint2 rrA = make_uint2(0u, 0u), rrB = rrA;
+        uint32_t dnA = 0u, dnB = 0u;  // position in the other layout
+        if (l8 < f.rows) {
+          rrA = __ldg(rrec + f.pos0 + l8);
+          dnA = (uint32_t)__ldg(dst_map + f.pos0 + l8);
+        }
+        if (l8 + 8 < f.rows) {
+          rrB = __ldg(rrec + f.pos0 + l8 + 8);
+          dnB = (uint32_t)__ldg(dst_map + f.pos0 + l8 + 8);
+        }
         double2 xo[kFibreMaxRows], acc[kFibreMaxRows];
 #pragma unroll
         for (int r = 0; r < kFibreMaxRows; ++r) {
@@ -870,20 +948,53 @@ __global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSm
             xo[r] = ldg128_stream(V + (size_t)(f.pos0 + r) * kTilePanel + 2 * l8, pol_first);
         }
         fibre_hops<NC>(a, f, w_me, max_hops, xl, acc);
+        {  // c V folded into the sum that p scales: V leaves the registers before the tail
+          const double c_over_p = a.cs / a.ps;
 #pragma unroll
-        for (int r = 0; r < kFibreMaxRows; ++r) {
-          if (r >= f.rows) break;
-          const int pos = f.pos0 + r;
-          const uint2 rr = __ldg(rrec + pos);
-          const int dst = __ldg(dst_map + pos);
-          double2 x1 = zero2;
-          if (a.rs != 0.0) x1 = ldg128(X1 + ((size_t)row0 + pos) * kTilePanel + 2 * l8);
-          row_hops<NC>(a, rr, xl, acc[r]);
-          double2 y;
-          y.x = fma(a.cs, xo[r].x, fma(a.rs, x1.x, a.ps * acc[r].x));
-          y.y = fma(a.cs, xo[r].y, fma(a.rs, x1.y, a.ps * acc[r].y));
-          stg128_hint(Pout + (size_t)dst * kTilePanel + 2 * l8, y, pol_first);
+          for (int r = 0; r < kFibreMaxRows; ++r) fma2(c_over_p, xo[r], acc[r]);
         }
+        uint2 rr_c;
+        uint32_t dn_c;
+        double2 x1_c;
+        auto fetch = [&](auto R, uint2& rr, uint32_t& dn, double2& x1) {
+          constexpr int RR = decltype(R)::value;
+          rr.x = row_bcast<RR>(rrA.x, rrB.x);
+          rr.y = row_bcast<RR>(rrA.y, rrB.y);
+          dn = row_bcast<RR>(dnA, dnB);
+          x1 = zero2;
+          if (RR < f.rows && a.rs != 0.0)
+            x1 = ldg128(X1 + ((size_t)row0 + f.pos0 + RR) * kTilePanel + 2 * l8);
+        };
+        fetch(std::integral_constant<int, 0>{}, rr_c, dn_c, x1_c);
+#define POLFED_FIBRE_ROW(R)                                                                    \
+  if (R < max_rows) {                                                                          \
+    uint2 rr_n = make_uint2(0u, 0u);                                                           \
+    uint32_t dn_n = 0u;                                                                        \
+    double2 x1_n = zero2;                                                                      \
+    if (R + 1 < max_rows)                                                                      \
+      fetch(std::integral_constant<int, (R + 1 < kFibreMaxRows ? R + 1 : 0)>{}, rr_n, dn_n, x1_n); \
+    if (R < f.rows) {                                                                          \
+      row_hops<NC>(a, rr_c, xl, acc[R]);                                                       \
+      double2 y;                                                                               \
+      y.x = fma(a.rs, x1_c.x, a.ps * acc[R].x);                                                \
+      y.y = fma(a.rs, x1_c.y, a.ps * acc[R].y);                                                \
+      stg128_hint(Pout + (size_t)dn_c * kTilePanel + 2 * l8, y, pol_first);                    \
+    }                                                                                          \
+    rr_c = rr_n;                                                                               \
+    dn_c = dn_n;                                                                               \
+    x1_c = x1_n;                                                                               \
+  }
+        POLFED_FIBRE_ROW(0)
+        POLFED_FIBRE_ROW(1)
+        POLFED_FIBRE_ROW(2)
+        POLFED_FIBRE_ROW(3)
+        POLFED_FIBRE_ROW(4)
+        POLFED_FIBRE_ROW(5)
+        POLFED_FIBRE_ROW(6)
+        POLFED_FIBRE_ROW(7)
+        POLFED_FIBRE_ROW(8)
+        POLFED_FIBRE_ROW(9)
+#undef POLFED_FIBRE_ROW
       }
       __syncthreads();  // all reads of the tile done before the next bulk copy
     }
