@@ -582,21 +582,6 @@ __device__ __forceinline__ void fma2(double c, const double2 x, double2& acc) {
   acc.y = fma(c, x.y, acc.y);
 }
 
-// The per-row records of a fibre (contiguous rows) are read row by row after the hops; ask for
-// their lines at the start of the chunk so that those reads hit L1.
-__device__ __forceinline__ void prefetch_l1(const void* p) {
-  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
-}
-__device__ __forceinline__ void fibre_prefetch(const void* base, int first, int count, int elem_bytes,
-                                               int l8) {
-  if (count <= 0) return;
-  const char* p0 = static_cast<const char*>(base) + (size_t)first * elem_bytes;
-  const char* p1 = p0 + (size_t)count * elem_bytes - 1;
-  const char* line = reinterpret_cast<const char*>((reinterpret_cast<uintptr_t>(p0) & ~(uintptr_t)127)) +
-                     128 * l8;
-  if (line <= p1) prefetch_l1(line);
-}
-
 // Per-row records of a fibre are loaded once per chunk, one row per lane (lane l8 holds rows l8
 // and l8 + 8), before the hops, and handed to the 8 lanes row by row with shuffles: no dependent
 // global load is left in the per-row tail.  R is a compile-time row number.
