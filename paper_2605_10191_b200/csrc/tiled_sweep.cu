@@ -80,7 +80,7 @@ struct D4 {
 
 __device__ __forceinline__ D4 ldg256(const double* p) {  // read-only data, default caching
   D4 r;
-  asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
                : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w)
                : "l"(p));
   return r;
