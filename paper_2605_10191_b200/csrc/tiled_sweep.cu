@@ -332,6 +332,21 @@ __device__ __forceinline__ void next_tile_prefetch(const SweepArgs& a, int tile,
 
 // THREADS = 512 with one CTA per SM for tiles that fill the shared memory, 256 with three CTAs
 // per SM (85 registers) for tiles of at most a third of it.
+// Same for a work item = (panel, tile) of the panel-major order of the row-record sweep.
+__device__ __forceinline__ void next_work_prefetch(const SweepArgs& a, int work_n,
+                                                   size_t panel_stride, int tid) {
+  if (work_n >= a.n_tiles * a.n_panels) return;
+  const int tile = work_n % a.n_tiles, npanel = work_n / a.n_tiles;
+  const int row0 = __ldg(a.tile_row0 + tile);
+  const unsigned bytes = (unsigned)(__ldg(a.tile_row0 + tile + 1) - row0) * 128u;
+  const unsigned at = (unsigned)tid * 2048u;
+  if (at < bytes)
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(
+                     a.X1 + npanel * panel_stride + (size_t)row0 * kTilePanel + at / 8),
+                 "r"(min(2048u, bytes - at))
+                 : "memory");
+}
+
 template <int NC, int MODE, int THREADS>
 __global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSmallCtas)
     tiled_sweep_kernel(const SweepArgs a) {
@@ -360,8 +375,10 @@ __global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSm
   const uint64_t pol_first = l2_policy_evict_first(), pol_last = l2_policy_evict_last();
 
   for (int it = 0;; ++it) {
-    const int tile = s_tile[it & 1];
-    if (tile >= a.n_tiles) break;
+    // work items in panel-major order: all tiles of panel 0, then panel 1 (half the live X in L2)
+    const int work = s_tile[it & 1];
+    if (work >= a.n_tiles * a.n_panels) break;
+    const int tile = work % a.n_tiles, panel_of_work = work / a.n_tiles;
     if (tid == 0) s_tile[(it + 1) & 1] = atomicAdd(a.counter, 1);  // read after later barriers
     const int row0 = __ldg(a.tile_row0 + tile);
     const int nrows = __ldg(a.tile_row0 + tile + 1) - row0;
@@ -373,7 +390,7 @@ __global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSm
     if (tid < 8) reinterpret_cast<double2*>(smem_raw)[nrows * 8 + tid] = zero2;  // the zero row
     __syncthreads();
 
-    for (int panel = 0; panel < a.n_panels; ++panel) {
+    for (int panel = panel_of_work; panel == panel_of_work; ++panel) {
 #ifdef POLFED_TILED_PROFILE
       long long t0 = clock64(), t1 = t0, t2 = t0, t3 = t0, t4 = t0;
 #endif
@@ -491,7 +508,7 @@ __global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSm
       uint4 rq_n = make_uint4(0u, 0u, 0u, 0u);
       if (base + slot < nrows) rq_n = __ldg(rec + (size_t)(base + slot) * 4 + q);
       if (MODE == MODE_STEP)
-        next_tile_prefetch(a, tile, s_tile[(it + 1) & 1], panel, panel_stride, tid);
+        next_work_prefetch(a, s_tile[(it + 1) & 1], panel_stride, tid);
       mbar_wait(&bar, parity);
       parity ^= 1u;
       PROF_CLOCK(t3);
