@@ -347,8 +347,11 @@ __device__ __forceinline__ void next_work_prefetch(const SweepArgs& a, int work_
                  : "memory");
 }
 
+// Register cap instead of launch bounds: 152 lets ptxas settle on 110 registers for the 384-thread
+// variant (4.62 ms per sweep on config 5; __launch_bounds__(384, 1): 115 registers, 4.69 ms;
+// cap 128: 4.67; cap 104: 5.5).
 template <int NC, int MODE, int THREADS>
-__global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSmallCtas)
+__global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
     tiled_sweep_kernel(const SweepArgs a) {
   constexpr int kIterRows = (THREADS / 32) * kRowsPerIter;  // rows per CTA pass (static loops)
   extern __shared__ __align__(128) unsigned char smem_raw[];  // (max_tile_rows + 1) x 128 B
