@@ -38,9 +38,10 @@ constexpr int kTileMaxCrossCoef = 15; // distinct |amplitude| values among the c
 constexpr uint32_t kCrossNone = 0xffffffffu;
 constexpr int kCrossPosBits = 26;     // cross word: bits 0-25 position, 26-29 amplitude, 31 sign
 constexpr int kTilePanel = 16;        // columns per panel: 128-byte rows, conflict-free in smem
-constexpr int kTileThreads = 384;       // one CTA per SM (tiles that fill the shared memory);
-                                        // measured on config 5: 256: 5.2, 384: 4.77, 512: 4.85,
-                                        // 640: 5.7 ms per sweep
+constexpr int kTileThreads = 448;       // one CTA per SM (tiles that fill the shared memory);
+                                        // measured on config 5 with the register cap of the sweep
+                                        // kernel, ms per sweep: 352: 4.62, 384: 4.61, 416: 4.53,
+                                        // 448: 4.51, 480: 4.56, 512: 4.67
 constexpr int kTileSmallThreads = 256;  // kTileSmallCtas CTAs per SM (small tiles)
 constexpr int kTileSmallCtas = 3;
 
