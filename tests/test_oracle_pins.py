@@ -274,6 +274,66 @@ def test_clenshaw_column_independence_and_linearity():
         assert np.array_equal(core.clenshaw(H, 0.2, 9.0, c, V[:, j:j + 1])[:, 0], W[:, j])
 
 
+# ---- sampled-row builder and single-step helper (full-size spot checks, cpu_baseline) ----
+
+@pytest.mark.parametrize("config,L", [(3, 14), (4, 9), (5, 14)])
+def test_build_csr_rows_equals_the_same_rows_of_build_csr(config, L):
+    # orc_build_csr_rows carries the full-size parity checks of configs 4-5 (tests/test_gpu_*.py)
+    # and bench.py's cpu_baseline: it must return exactly the rows of the full assembly (O2,
+    # PAPER.md:858-861 Eq. 54, 939-946 Eq. 67), whatever the order of the requested rows.
+    w = workloads.make_workload(config, L_override=L)
+    st, H = core.hamiltonian(w)
+    D = H.n
+    rng = np.random.default_rng(17 + config)
+    rows = np.concatenate([[0, D - 1, D - 1, 0, D // 2], rng.integers(0, D, 400),
+                           np.arange(D - 5, D), np.arange(7)[::-1]]).astype(np.int64)
+    sub = core.build_csr_rows(st, rows, w.terms, w.dot_bits, w.dot_dense)
+    assert sub.n == rows.size and sub.row_ptr[0] == 0
+    assert np.array_equal(np.diff(sub.row_ptr), np.diff(H.row_ptr)[rows])
+    assert sub.nnz == int(np.diff(H.row_ptr)[rows].sum())
+    for k, r in enumerate(rows):
+        lo, hi = H.row_ptr[r], H.row_ptr[r + 1]
+        slo, shi = sub.row_ptr[k], sub.row_ptr[k + 1]
+        assert np.array_equal(sub.col[slo:shi], H.col[lo:hi])
+        assert np.array_equal(sub.val[slo:shi].view(np.int64), H.val[lo:hi].view(np.int64))
+    # and the product on the mini-CSR is the corresponding rows of the full product
+    X = rng.standard_normal((D, 3))
+    assert np.array_equal(core.spmm(sub, X), core.spmm(H, X)[rows])
+
+
+def test_build_csr_rows_empty_selection():
+    w = workloads.make_workload(5, L_override=10)
+    st, _ = core.hamiltonian(w)
+    sub = core.build_csr_rows(st, np.zeros(0, np.int64), w.terms)
+    assert sub.n == 0 and sub.nnz == 0 and sub.row_ptr.tolist() == [0]
+
+
+@pytest.mark.parametrize("K", [1, 2, 3, 17, 120])
+def test_clenshaw_step_chain_reproduces_clenshaw(K):
+    # the timed cpu_baseline calls orc_clenshaw_step; K-1 of them with the buffer swap of Fig. 5
+    # must give the b_1, b_2 of orc_clenshaw (Eq. 51) to the last bit, and the
+    # final line W = c_0 V + H~ b_1 - b_2 must then reproduce its W.
+    A, H = random_symmetric_csr(60, 0.2, 40 + K)
+    ev = np.linalg.eigvalsh(A)
+    a, b = cheb.rescale_params(ev[0], ev[-1], 0.01)
+    rng = np.random.default_rng(K)
+    c = rng.standard_normal(K + 1)
+    V = rng.standard_normal((60, 4))
+    B1 = c[K] * V                      # b_K = c_K V (b_{K+1} = b_{K+2} = 0)
+    B2 = np.zeros_like(V)
+    T = np.empty_like(V)
+    for k in range(K - 1, 0, -1):
+        core.clenshaw_step(H, a, b, float(c[k]), V, B1, B2, T)   # B2 <- c_k V + 2 H~ B1 - B2
+        B1, B2 = B2, B1
+    W = c[0] * V + core.rescaled_apply(H, a, b, B1) - B2
+    want = core.clenshaw(H, a, b, c, V)
+    assert np.array_equal(W.view(np.int64), want.view(np.int64))
+    # and against the spectral definition, so that the chain is pinned to something else too
+    evv, U = np.linalg.eigh(A)
+    truth = U @ (npcheb.chebval((evv - a) / b, c)[:, None] * (U.T @ V))
+    assert np.linalg.norm(W - truth) <= 1e-12 * max(1.0, np.linalg.norm(truth)) * (K + 1)
+
+
 # ---- order rule (Eq. 40-42) ------------------------------------------------------
 
 def test_order_rule_constant_and_cutoff():
@@ -332,6 +392,43 @@ def test_gaussian_and_kpm_dos_integrate_to_dimension_and_track_histogram():
     centers = 0.5 * (edges[1:] + edges[:-1])
     kc = cheb.kpm_dos(centers, exact, cheb.jackson_kernel(75)) * (edges[1] - edges[0])
     assert np.max(np.abs(kc - hist)) < 0.25 * hist.max()
+
+
+@pytest.mark.parametrize("N", [8, 75, 200])
+def test_jackson_kernel_is_the_autocorrelation_of_its_optimal_weights(N):
+    # Eq. (39)/(84).  The Jackson kernel is the solution of a
+    # variational problem (narrowest positive kernel): g_n = sum_{v=0}^{N-1-n} a_v a_{v+n} with
+    # a_v proportional to sin(pi (v+1)/(N+1)), normalised to g_0 = 1.  That sum is an object
+    # independent of the closed form the oracle types in.
+    g = cheb.jackson_kernel(N)
+    assert g.shape == (N,)
+    a = np.sin(np.pi * (np.arange(N) + 1) / (N + 1))
+    a /= np.sqrt(np.sum(a * a))
+    want = np.array([np.dot(a[:N - n], a[n:]) for n in range(N)])
+    assert np.max(np.abs(g - want)) < 1e-13
+    assert abs(g[0] - 1.0) < 1e-15 and np.all(np.diff(g) < 0) and 0 < g[-1] < 2.0 / N
+    # positivity of the kernel polynomial (a delta function smeared with g_n stays >= 0)
+    x = np.cos(np.linspace(0.0, np.pi, 4001))
+    n = np.arange(N)
+    for y in (0.0, 0.37, -0.9):
+        Ty = np.cos(n * np.arccos(y))
+        series = g[0] + 2.0 * (np.cos(np.outer(np.arccos(x), n[1:])) @ (g[1:] * Ty[1:]))
+        assert series.min() > -1e-10
+
+
+def test_gaussian_dos_is_centred_at_mu_with_width_gamma():
+    # Eq. (34): maximum D/(sqrt(2 pi) Gamma) at E = mu, symmetric about it,
+    # full width at half maximum 2 sqrt(2 ln 2) Gamma.
+    D, mu, Gamma = 924.0, 0.31, 0.27
+    E = np.linspace(mu - 2.0, mu + 2.0, 400001)
+    rho = cheb.gaussian_dos(E, D, mu, Gamma)
+    assert abs(E[np.argmax(rho)] - mu) < 2e-5
+    assert abs(rho.max() - D / (math.sqrt(2 * math.pi) * Gamma)) < 1e-9 * D
+    assert np.allclose(cheb.gaussian_dos(mu + 0.4, D, mu, Gamma), cheb.gaussian_dos(mu - 0.4, D, mu, Gamma),
+                       rtol=1e-14)
+    above = E[rho >= 0.5 * rho.max()]
+    assert abs((above[-1] - above[0]) - 2.0 * math.sqrt(2.0 * math.log(2.0)) * Gamma) < 5e-5
+    assert abs(np.sum(rho) * (E[1] - E[0]) - D) < 1e-6 * D
 
 
 # ---- Lanczos ----------------------------------------------------------------------
