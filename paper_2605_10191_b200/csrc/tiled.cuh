@@ -45,19 +45,6 @@ constexpr int kTileThreads = 448;       // one CTA per SM (tiles that fill the s
 constexpr int kTileSmallThreads = 256;  // kTileSmallCtas CTAs per SM (small tiles)
 constexpr int kTileSmallCtas = 3;
 
-// Fibre mode ("fibres"): the rows of a tile that differ only on the lowest g sites
-// -- a fibre, at most C(5,2) = 10 rows -- are stored together and owned by 8 lanes (16 bytes of
-// every row each), which hold them in registers.  Hops among the low g sites are a dense matrix
-// applied in registers; hops among the other tile sites map a fibre onto one other fibre (one
-// record entry for all its rows); only hops between the two groups are per row.
-constexpr int kFibreMaxSites = 5;
-constexpr int kFibreMaxRows = 10;
-constexpr int kFibreRecWords = 8;   // header + 7 words of two fibre-level neighbours each
-constexpr int kFibreMaxHops = 14;
-constexpr int kFibreRowHops = 3;    // per-row neighbours (two 32-bit words per row)
-constexpr int kFibreDense = 252;    // sum_j C(5,j)^2 entries of the in-fibre matrices
-constexpr int kFibresPerChunk = 4;  // a warp works on four fibres of the same sector
-
 // Record of one class row (position order), kTileRecWords words:
 //   word 0      in-tile degree
 //   words 1-12  two neighbours per word:
@@ -80,11 +67,9 @@ struct TiledLayout {
   int32_t* d_from_natural = nullptr;  // [n] position of the caller's row
   double coef[kTileMaxCoef] = {0, 0, 0, 0};
   int n_coef = 0;
-  // fibre mode
-  uint32_t* d_fibre_rec = nullptr;    // [fibres of all classes][kFibreRecWords]
-  uint32_t* d_row_rec = nullptr;      // [2^m][2] per-row neighbours, class blocks in position order
-  double dense[kFibreDense] = {};     // in-fibre matrices, sector j at dense_off[j], [r][c]
 };
+
+struct SectorPlan;  // sector.cuh
 
 struct TiledPlan {
   int n_sites = 0, n_up = 0, m = 0;
@@ -93,15 +78,10 @@ struct TiledPlan {
   int max_tile_rows = 0;
   int grid = 0;                     // persistent CTAs
   int threads = kTileThreads;       // threads per CTA (kTileThreads or kTileSmallThreads)
-  int fibre_g = 0;                  // > 0: fibre mode with g low sites per fibre
-  int fibre_size[kFibreMaxSites + 1] = {};   // rows of a fibre with j particles on the g sites
-  int dense_off[kFibreMaxSites + 1] = {};
-  int32_t* d_tile_fib0 = nullptr;   // [n_tiles] first fibre record of the tile's class
-  int32_t* d_tile_chunks = nullptr; // [n_tiles] chunks (of kFibresPerChunk fibres) of the class
   size_t smem_bytes = 0;
   int32_t* d_tile_row0 = nullptr;   // [n_tiles + 1]
   int32_t* d_tile_rec0 = nullptr;   // [n_tiles] first record row of the tile's class
-  int* d_counter = nullptr;         // dynamic tile scheduler
+  SectorPlan* sector = nullptr;     // the sector sweep takes over (uniform NN/NNN bonds)
   TiledLayout lay[2];
 };
 

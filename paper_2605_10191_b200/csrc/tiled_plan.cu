@@ -8,6 +8,7 @@
 #include <new>
 
 #include "combinadic.cuh"
+#include "sector.cuh"
 #include "tiled.cuh"
 
 namespace polfed {
@@ -222,173 +223,156 @@ int build_records(int m, const std::vector<DevTerm>& low, TiledLayout* lay,
   return POLFED_OK;
 }
 
-// ---- fibre mode ------------------------------------------------------------------------------
-struct FibreTables {
-  std::vector<uint32_t> frec;      // fibre records of all classes (padded per sector)
-  std::vector<uint32_t> rrec;      // [2^m][2] row records by class_off[k] + position
-  std::vector<int32_t> inv_sigma;  // class_off[k] + ascending class rank -> position in class
-  std::vector<int> class_fib0, class_chunks;  // per class k
-};
 
-// JW sign (1 = negative) and applicability of a hop term on the m-bit configuration l.
-inline bool hop_applies(const DevTerm& t, uint32_t l, uint32_t* l2, uint32_t* sign) {
+// ---- sector sweep (sector.cuh) ---------------------------------------------------------------
+// JW sign (1 = negative, the sign of amp not included) and applicability of a hop term on the
+// m-bit configuration l.
+inline bool hop_applies(const DevTerm& t, uint32_t l, uint32_t* l2, uint32_t* jw_sign) {
   const int i = t.i, j = t.j;
   if (((l >> i) & 1u) == ((l >> j) & 1u)) return false;
   *l2 = l ^ (1u << i) ^ (1u << j);
-  uint32_t sg = t.amp < 0 ? 1u : 0u;
+  uint32_t sg = 0u;
   if (t.kind == POLFED_TERM_HOPJW) {
     const int lo = std::min(i, j), hi = std::max(i, j);
     const uint32_t between = ((1u << hi) - 1u) & ~((2u << lo) - 1u);
-    sg ^= (uint32_t)__builtin_popcount(l & between) & 1u;
+    sg = (uint32_t)__builtin_popcount(l & between) & 1u;
   }
-  *sign = sg;
+  *jw_sign = sg;
   return true;
 }
 
-// Rank of the g-bit configuration c among the configurations of equal popcount (ascending).
-inline int sector_rank(uint32_t c) { return (int)class_rank(c); }
-
-// Builds the fibre-mode tables of one layout; returns POLFED_EINVAL (with *fits = false) when a
-// limit of the record formats is exceeded, so that the caller can fall back to row records.
-int build_fibres(int m, int g, const std::vector<DevTerm>& low, TiledLayout* lay, TiledPlan* plan,
-                 const std::vector<int>& class_off, FibreTables* out, bool* fits) {
-  *fits = false;
-  lay->n_coef = 0;
-  std::vector<int> cls(low.size(), -1), where(low.size(), 0);  // 0 in-fibre, 1 fibre-level, 2 row
-  for (size_t t = 0; t < low.size(); ++t) {
-    const double mag = std::fabs(low[t].amp);
-    if (mag == 0.0) continue;
-    const int a = std::min(low[t].i, low[t].j), b = std::max(low[t].i, low[t].j);
-    where[t] = b < g ? 0 : (a >= g ? 1 : 2);
-    cls[t] = 0;
-    if (where[t] == 0) continue;  // in-fibre amplitudes go into the dense matrices as they are
-    int c = 0;
-    while (c < lay->n_coef && lay->coef[c] != mag) ++c;
-    if (c == lay->n_coef) {
-      if (c == kTileMaxCoef) return POLFED_OK;  // does not fit
-      lay->coef[lay->n_coef++] = mag;
-    }
-    cls[t] = c;
-  }
-  // sector sizes and the in-fibre matrices
-  int off = 0;
-  for (int j = 0; j <= kFibreMaxSites; ++j) {
-    plan->fibre_size[j] = j <= g ? (int)host_binom(g, j) : 0;
-    plan->dense_off[j] = off;
-    off += plan->fibre_size[j] * plan->fibre_size[j];
-  }
-  for (double& d : lay->dense) d = 0.0;
-  for (uint32_t c = 0; c < (1u << g); ++c) {
-    const int j = __builtin_popcount(c), f = plan->fibre_size[j];
-    for (size_t t = 0; t < low.size(); ++t) {
-      if (cls[t] < 0 || where[t] != 0) continue;
-      uint32_t c2, sg;
-      if (!hop_applies(low[t], c, &c2, &sg)) continue;
-      // row = c (output), column = c2 (input); the term is symmetric, amplitude |amp| with sign
-      lay->dense[plan->dense_off[j] + sector_rank(c) * f + sector_rank(c2)] +=
-          (sg ? -1.0 : 1.0) * std::fabs(low[t].amp);
+// True when the tile-local hops of a layout are exactly one bond (i, i+1) for every i < m - 1
+// with one amplitude t1 and either no or one bond (i, i+2) for every i < m - 2 with one
+// amplitude t2 (all HOPJW: jw, or all EXCH).
+bool sector_pattern(int m, const std::vector<DevTerm>& low, double* t1, double* t2, bool* nnn,
+                    bool* jw) {
+  std::vector<int> cnt1(m, 0), cnt2(m, 0);
+  int n_jw = 0, n_ex = 0, n1 = 0, n2 = 0;
+  *t1 = *t2 = 0.0;
+  for (const DevTerm& t : low) {
+    if (t.amp == 0.0) continue;
+    const int lo = std::min(t.i, t.j), d = std::max(t.i, t.j) - lo;
+    if (d == 1) {
+      if (n1++ == 0) *t1 = t.amp;
+      if (t.amp != *t1 || ++cnt1[lo] > 1) return false;
+    } else if (d == 2) {
+      if (n2++ == 0) *t2 = t.amp;
+      if (t.amp != *t2 || ++cnt2[lo] > 1) return false;
+      (t.kind == POLFED_TERM_HOPJW ? n_jw : n_ex)++;
+    } else {
+      return false;
     }
   }
+  if (n1 != m - 1) return false;
+  if (n2 != 0 && (n2 != m - 2 || (n_jw != 0 && n_ex != 0))) return false;
+  *nnn = n2 != 0;
+  *jw = n_jw != 0;
+  return true;
+}
 
-  const size_t n_cfg = (size_t)1 << m;
-  const uint32_t n_up_cfg = 1u << (m - g);
-  out->inv_sigma.assign(n_cfg, 0);
-  out->rrec.assign(n_cfg * 2, 0u);
-  out->frec.clear();
-  out->class_fib0.assign(m + 1, 0);
-  out->class_chunks.assign(m + 1, 0);
+struct SectorHost {
+  std::vector<int32_t> inv_sigma;  // class_off[k] + ascending class rank -> position in class
+  std::vector<uint64_t> xg;        // class_off[k] + position -> three cross-group entries
+};
 
-  struct Fibre {
-    uint32_t u;
-    int j;
-    std::vector<Entry> hops;  // nbr = partner upper configuration (resolved to a position later)
-  };
+// Geometry shared by both layouts: sector bases, fibre pitches, work units.
+void sector_geometry(int m, bool pad, SectorPlan* sp, std::vector<uint16_t>* units) {
+  const int g1 = m / 2, g2 = m - g1;
+  sp->m = m;
+  sp->g1 = g1;
+  sp->g2 = g2;
+  SectorTables& T = sp->tab;
+  for (int j = 0; j <= kSecMaxG; ++j) {
+    T.n1[j] = j <= g1 ? (short)host_binom(g1, j) : 0;
+    T.n2[j] = j <= g2 ? (short)host_binom(g2, j) : 0;
+    T.n1p[j] = (short)((pad && T.n1[j] > 1 && T.n1[j] % 2 == 0) ? T.n1[j] + 1 : T.n1[j]);
+  }
+  units->assign((size_t)2 * (m + 1) * kSecMaxUnits, 0);
+  sp->max_rows_p = 1;
   for (int k = 0; k <= m; ++k) {
-    std::vector<Fibre> fibres;
-    for (uint32_t u = 0; u < n_up_cfg; ++u) {
-      const int j = k - __builtin_popcount(u);
-      if (j < 0 || j > g) continue;
-      Fibre fb{u, j, {}};
-      for (size_t t = 0; t < low.size(); ++t) {
-        if (cls[t] < 0 || where[t] != 1) continue;
-        uint32_t l2, sg;
-        if (!hop_applies(low[t], u << g, &l2, &sg)) continue;
-        fb.hops.push_back(Entry{l2 >> g, (uint32_t)cls[t], sg});
-      }
-      if ((int)fb.hops.size() > kFibreMaxHops) return POLFED_OK;
-      fibres.push_back(fb);
+    int pos = 0, row = 0;
+    struct U { int cost; uint16_t code; };
+    std::vector<U> u1, u2;
+    for (int j1 = std::max(0, k - g2); j1 <= std::min(g1, k); ++j1) {
+      const int n1 = T.n1[j1], n2 = T.n2[k - j1];
+      T.sbase[k][j1] = (short)pos;
+      T.srow[k][j1] = (short)row;
+      pos += n1 * n2;
+      row += T.n1p[j1] * n2;
+      for (int q = 0; q * kSecGroups < n2; ++q) u1.push_back(U{n1, (uint16_t)(j1 | (q << 3))});
+      for (int q = 0; q * kSecGroups < n1; ++q) u2.push_back(U{n2, (uint16_t)(j1 | (q << 3))});
     }
-    // large sectors first, then falling fibre degree: the chunks a CTA claims last are small
-    std::stable_sort(fibres.begin(), fibres.end(), [&](const Fibre& a, const Fibre& b) {
-      const int fa = plan->fibre_size[a.j], fbs = plan->fibre_size[b.j];
-      if (fa != fbs) return fa > fbs;
-      if (a.j != b.j) return a.j < b.j;
-      return a.hops.size() > b.hops.size();
-    });
-    // positions: fibres in this order, rows of a fibre ascending in the low configuration
-    std::vector<int> fibre_pos0(n_up_cfg, -1);
-    int32_t* inv = out->inv_sigma.data() + class_off[k];
-    int pos = 0;
-    for (const Fibre& fb : fibres) {
-      fibre_pos0[fb.u] = pos;
-      for (uint32_t c = 0; c < (1u << g); ++c) {
-        if (__builtin_popcount(c) != fb.j) continue;
-        inv[class_rank((fb.u << g) | c)] = pos++;
-      }
-    }
-    if (pos != class_off[k + 1] - class_off[k]) return fail(POLFED_ECUDA, "fibre tables: bad class");
-    // fibre records, padded so that a chunk of kFibresPerChunk fibres never mixes sectors
-    out->class_fib0[k] = (int)(out->frec.size() / kFibreRecWords);
-    auto emit = [&](const Fibre* fb) {
-      uint32_t w[kFibreRecWords] = {0, 0, 0, 0, 0, 0, 0, 0};
-      if (fb) {
-        w[0] = (uint32_t)fibre_pos0[fb->u] | ((uint32_t)fb->j << 11) |
-               ((uint32_t)fb->hops.size() << 14) | (1u << 18);
-        for (size_t e = 0; e < fb->hops.size(); ++e) {
-          const uint32_t p0 = (uint32_t)fibre_pos0[fb->hops[e].nbr];
-          uint32_t& word = w[1 + (e >> 1)];
-          if ((e & 1) == 0) word |= (p0 << 7) | fb->hops[e].cls | (fb->hops[e].sign << 30);
-          else word |= (p0 << 18) | (fb->hops[e].cls << 2) | (fb->hops[e].sign << 31);
-        }
-      }
-      out->frec.insert(out->frec.end(), w, w + kFibreRecWords);
-    };
-    size_t at = 0;
-    while (at < fibres.size()) {
-      size_t end = at;
-      while (end < fibres.size() && fibres[end].j == fibres[at].j) ++end;
-      for (size_t f = at; f < end; ++f) emit(&fibres[f]);
-      for (size_t f = end - at; f % kFibresPerChunk; ++f) emit(nullptr);
-      at = end;
-    }
-    out->class_chunks[k] =
-        (int)(out->frec.size() / kFibreRecWords - out->class_fib0[k]) / kFibresPerChunk;
-    // row records: hops between the low g sites and the rest
-    for (const Fibre& fb : fibres)
-      for (uint32_t c = 0; c < (1u << g); ++c) {
-        if (__builtin_popcount(c) != fb.j) continue;
-        const uint32_t l = (fb.u << g) | c;
-        uint32_t ent[kFibreRowHops], cnt = 0;
-        for (size_t t = 0; t < low.size(); ++t) {
-          if (cls[t] < 0 || where[t] != 2) continue;
-          uint32_t l2, sg;
-          if (!hop_applies(low[t], l, &l2, &sg)) continue;
-          if (cnt == kFibreRowHops) return POLFED_OK;
-          ent[cnt++] = (uint32_t)inv[class_rank(l2)] | ((uint32_t)cls[t] << 11) | (sg << 13);
-        }
-        uint32_t* w = out->rrec.data() + ((size_t)class_off[k] + inv[class_rank(l)]) * 2;
-        w[0] = (cnt > 0 ? ent[0] : 0u) | ((cnt > 1 ? ent[1] : 0u) << 14) | (cnt << 28);
-        w[1] = cnt > 2 ? ent[2] : 0u;
-      }
+    T.rows_p[k] = (short)row;
+    sp->max_rows_p = std::max(sp->max_rows_p, row);
+    auto by_cost = [](const U& a, const U& b) { return a.cost > b.cost; };
+    std::stable_sort(u1.begin(), u1.end(), by_cost);
+    std::stable_sort(u2.begin(), u2.end(), by_cost);
+    T.n_units[0][k] = (short)u1.size();
+    T.n_units[1][k] = (short)u2.size();
+    for (size_t i = 0; i < u1.size(); ++i) (*units)[(size_t)k * kSecMaxUnits + i] = u1[i].code;
+    for (size_t i = 0; i < u2.size(); ++i)
+      (*units)[(size_t)(m + 1 + k) * kSecMaxUnits + i] = u2[i].code;
   }
-  *fits = true;
-  return POLFED_OK;
+}
+
+// Sector order of the class rows and the cross-group entries of one layout.
+void sector_tables(const SectorPlan& sp, const std::vector<DevTerm>& low,
+                   const std::vector<int>& class_off, SectorHost* out) {
+  const int m = sp.m, g1 = sp.g1;
+  const SectorTables& T = sp.tab;
+  const size_t n_cfg = (size_t)1 << m;
+  out->inv_sigma.assign(n_cfg, 0);
+  out->xg.assign(n_cfg, 0ull);
+  auto locate = [&](uint32_t l, int* pos, int* srow) {
+    const int k = __builtin_popcount(l);
+    const uint32_t c1 = l & ((1u << g1) - 1u), c2 = l >> g1;
+    const int j1 = __builtin_popcount(c1);
+    const int i1 = (int)class_rank(c1), i2 = (int)class_rank(c2);
+    *pos = T.sbase[k][j1] + i2 * T.n1[j1] + i1;
+    *srow = T.srow[k][j1] + i2 * T.n1p[j1] + i1;
+  };
+  for (uint32_t l = 0; l < n_cfg; ++l) {
+    const int k = __builtin_popcount(l);
+    int pos, srow;
+    locate(l, &pos, &srow);
+    out->inv_sigma[(size_t)class_off[k] + class_rank(l)] = pos;
+    uint64_t rec = (uint64_t)srow << 48;  // the row's own shared-memory row
+    for (const DevTerm& t : low) {
+      const int lo = std::min(t.i, t.j), hi = std::max(t.i, t.j);
+      if (t.amp == 0.0 || !(lo < g1 && hi >= g1)) continue;
+      uint32_t l2, sg;
+      if (!hop_applies(t, l, &l2, &sg)) continue;
+      int pos2, srow2;
+      locate(l2, &pos2, &srow2);
+      // slot 0: the (g1-1, g1) bond (t1); slot 1: (g1-2, g1), slot 2: (g1-1, g1+1) (t2)
+      const int slot = hi - lo == 1 ? 0 : (lo == g1 - 2 ? 1 : 2);
+      rec |= ((uint64_t)srow2 | kXgValid | (sg ? kXgNeg : 0u)) << (16 * slot);
+    }
+    out->xg[(size_t)class_off[k] + pos] = rec;
+  }
+}
+
+// side (4 words) + cross-group entries + diagonal -> the 32-byte row record of sector.cuh.
+__global__ void __launch_bounds__(256) sector_meta_kernel(const int32_t* __restrict__ tile_row0,
+                                                          const int32_t* __restrict__ tile_rec0,
+                                                          const uint4* __restrict__ side,
+                                                          const double* __restrict__ diag,
+                                                          const unsigned long long* __restrict__ xg,
+                                                          uint4* __restrict__ meta) {
+  const int row0 = tile_row0[blockIdx.x], nrows = tile_row0[blockIdx.x + 1] - row0;
+  const int rec0 = tile_rec0[blockIdx.x];
+  for (int i = threadIdx.x; i < nrows; i += blockDim.x) {
+    const size_t p = (size_t)row0 + i;
+    const uint4 sd = side[p];
+    const unsigned long long x = xg[rec0 + i];
+    const long long d = __double_as_longlong(diag[p]);
+    meta[2 * p] = make_uint4(sd.x, (uint32_t)x, (uint32_t)(x >> 32), sd.y);
+    meta[2 * p + 1] = make_uint4(sd.z, sd.w, (uint32_t)d, (uint32_t)((unsigned long long)d >> 32));
+  }
 }
 
 void free_layout(TiledLayout& l) {
   cudaFree(l.d_records);
-  cudaFree(l.d_fibre_rec);
-  cudaFree(l.d_row_rec);
   cudaFree(l.d_diag);
   cudaFree(l.d_side);
   cudaFree(l.d_to_other);
@@ -417,9 +401,7 @@ void destroy_tiled_plan(TiledPlan* p) {
   for (auto& l : p->lay) free_layout(l);
   cudaFree(p->d_tile_row0);
   cudaFree(p->d_tile_rec0);
-  cudaFree(p->d_tile_fib0);
-  cudaFree(p->d_tile_chunks);
-  cudaFree(p->d_counter);
+  destroy_sector_plan(p->sector);
   delete p;
 }
 
@@ -493,6 +475,39 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
   rc = upload(&p->d_tile_rec0, rec0);
   if (rc) return rc;
 
+  // The sector sweep takes over when both layouts have uniform NN (+ NNN) bonds inside their
+  // tiles, at most three hops cross the cut and a kernel exists for this tile size.
+  SectorHost sh[2];
+  {
+    double t1[2], t2[2];
+    bool nnn[2], jw[2];
+    int cross_terms = 0;
+    for (const DevTerm& t : dm[0]) cross_terms += off_diagonal(t.kind) && t.amp != 0.0;
+    const bool pat = m >= 2 && cross_terms <= 3 &&
+                     sector_pattern(m, low[0], &t1[0], &t2[0], &nnn[0], &jw[0]) &&
+                     sector_pattern(m, low[1], &t1[1], &t2[1], &nnn[1], &jw[1]) &&
+                     nnn[0] == nnn[1] && (!nnn[0] || jw[0] == jw[1]) &&
+                     sector_m_supported(m, nnn[0], jw[0]);
+    if (pat) {
+      SectorPlan* sp = new (std::nothrow) SectorPlan;
+      if (!sp) return fail(POLFED_ENOMEM, "tiled format: host allocation failed");
+      p->sector = sp;
+      sp->nnn = nnn[0];
+      sp->jw = nnn[0] && jw[0];
+      std::vector<uint16_t> units;
+      sector_geometry(m, /*pad=*/getenv("POLFED_SECTOR_PAD") != nullptr, sp, &units);
+      for (int l = 0; l < 2; ++l) {
+        sp->lay[l].t1 = t1[l];
+        sp->lay[l].t2 = t2[l];
+        sector_tables(*sp, low[l], class_off, &sh[l]);
+      }
+      rc = upload(&sp->d_units, units);
+      if (rc) return rc;
+      rc = upload(&sp->d_tile_class, tile_class);
+      if (rc) return rc;
+    }
+  }
+
   DeviceTemp tmp;
   int32_t* d_pi = nullptr;
   int32_t* d_pos[2] = {nullptr, nullptr};
@@ -508,42 +523,12 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
                 (long long)n, kCrossPosBits);
   const unsigned row_grid = (unsigned)((n + 255) / 256);
 
-  // Fibre mode (opt-in) where the record formats allow it, else row records: g low sites per fibre.
-  FibreTables ft[2];
-  // Experimental: a third fewer shared-memory wavefronts but slower so far, so
-  // the row-record sweep stays the default; POLFED_TILED_FIBRE=1 at build time selects it.
-  int g = getenv("POLFED_TILED_FIBRE") ? std::min(kFibreMaxSites, m - 1) : 0;
-  if (g >= 1) {
-    for (int l = 0; l < 2 && g >= 1; ++l) {
-      bool fits = false;
-      rc = build_fibres(m, g, low[l], &p->lay[l], p, class_off, &ft[l], &fits);
-      if (rc) return rc;
-      if (!fits) g = 0;
-    }
-  }
-  p->fibre_g = g >= 1 ? g : 0;
-  if (p->fibre_g) {
-    std::vector<int32_t> fib0, chunks;
-    for (int k : tile_class) {
-      fib0.push_back(ft[0].class_fib0[k]);
-      chunks.push_back(ft[0].class_chunks[k]);
-    }
-    rc = upload(&p->d_tile_fib0, fib0);
-    if (rc) return rc;
-    rc = upload(&p->d_tile_chunks, chunks);
-    if (rc) return rc;
-  }
-
   for (int l = 0; l < 2; ++l) {
     TiledLayout& lay = p->lay[l];
     std::vector<uint32_t> rec;
     std::vector<int32_t> inv_sigma;
-    if (p->fibre_g) {
-      inv_sigma = ft[l].inv_sigma;
-      rc = upload(&lay.d_fibre_rec, ft[l].frec);
-      if (rc) return rc;
-      rc = upload(&lay.d_row_rec, ft[l].rrec);
-      if (rc) return rc;
+    if (p->sector) {
+      inv_sigma = sh[l].inv_sigma;
     } else {
       rc = build_records(m, low[l], &lay, &rec, &inv_sigma, class_off);
       if (rc) return rc;
@@ -627,10 +612,36 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
                                           p->lay[1].side_words);
     POLFED_LAUNCH_CHECK("maps_kernel");
   }
-  POLFED_CUDA(cudaMalloc(&p->d_counter, sizeof(int)));
-  POLFED_CUDA(cudaMemsetAsync(p->d_counter, 0, sizeof(int), st));
   POLFED_CUDA(cudaStreamSynchronize(st));
-  rc = tiled_configure_launch(p);
+  if (p->sector) {
+    SectorPlan* sp = p->sector;
+    for (int l = 0; l < 2; ++l) {
+      TiledLayout& lay = p->lay[l];
+      if (lay.side_words != 4) return fail(POLFED_ECUDA, "sector sweep: wide cut");
+      unsigned long long* d_xg = nullptr;
+      POLFED_CUDA(tmp.alloc(&d_xg, sh[l].xg.size()));
+      POLFED_CUDA(cudaMemcpyAsync(d_xg, sh[l].xg.data(), sizeof(uint64_t) * sh[l].xg.size(),
+                                  cudaMemcpyHostToDevice, st));
+      POLFED_CUDA(cudaMalloc(&sp->lay[l].d_meta, sizeof(uint4) * 2 * n_alloc));
+      if (p->n_tiles > 0) {
+        sector_meta_kernel<<<(unsigned)p->n_tiles, 256, 0, st>>>(
+            p->d_tile_row0, p->d_tile_rec0, reinterpret_cast<const uint4*>(lay.d_side), lay.d_diag,
+            d_xg, sp->lay[l].d_meta);
+        POLFED_LAUNCH_CHECK("sector_meta_kernel");
+      }
+      POLFED_CUDA(cudaStreamSynchronize(st));
+      // the row records carry these now
+      cudaFree(lay.d_side);
+      cudaFree(lay.d_diag);
+      cudaFree(lay.d_to_other);
+      lay.d_side = nullptr;
+      lay.d_diag = nullptr;
+      lay.d_to_other = nullptr;
+    }
+    rc = sector_configure_launch(p, sp);
+  } else {
+    rc = tiled_configure_launch(p);
+  }
   if (rc) return rc;
   guard.p = nullptr;
   *out = p;

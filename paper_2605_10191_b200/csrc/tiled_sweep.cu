@@ -12,6 +12,7 @@
 #include <cstdlib>
 #include <type_traits>
 
+#include "sector.cuh"
 #include "tiled.cuh"
 
 namespace polfed {
@@ -46,32 +47,6 @@ struct SweepArgs {
   double pf;              // finishing scalar p_k
   double ps, qs, rs, cs;  // starting scalars of step k-1
   int mode;
-  // fibre mode (tiled.cuh)
-  const uint32_t* fibre_rec;
-  const uint32_t* row_rec;
-  const int32_t* tile_fib0;
-  const int32_t* tile_chunks;
-  int fibre_size[kFibreMaxSites + 1];
-  int dense_off[kFibreMaxSites + 1];
-  double dense[kFibreDense];
-#ifdef POLFED_TILED_PROFILE
-  int skip;                  // POLFED_TILED_SKIP: parts of the sweep left out (timing only)
-  unsigned long long* prof;  // per CTA: cycles in tile load / phase 2 / reload / phase 3, count
-#endif
-};
-
-// Developer build (-DPOLFED_TILED_PROFILE, see build.py): per-phase cycle counters and a mask that
-// leaves parts of the sweep out, for the ablation in profiles/r01_tiled_phase_ablation.md.
-#ifdef POLFED_TILED_PROFILE
-#define PROF_SKIP(bit) ((a.skip & (bit)) != 0)
-#define PROF_CLOCK(var) var = clock64()
-#else
-#define PROF_SKIP(bit) false
-#define PROF_CLOCK(var)
-#endif
-enum {
-  SKIP_HOPS2 = 1, SKIP_HOPS3 = 2, SKIP_PK = 4, SKIP_CROSS = 8, SKIP_BOUT = 16, SKIP_SCRATCH = 32,
-  SKIP_X1 = 64, SKIP_V = 128, SKIP_POUT = 256
 };
 
 struct D4 {
@@ -311,25 +286,6 @@ __device__ __forceinline__ int grab_chunk(int* counter, int lane) {
   return __shfl_sync(0xffffffffu, v, 0);
 }
 
-// Ask L2 for the tile panel of b_{k+1} this CTA loads next, while phase 3 of the current one runs.
-__device__ __forceinline__ void next_tile_prefetch(const SweepArgs& a, int tile, int tile_n,
-                                                   int panel, size_t panel_stride, int tid) {
-  int npanel = panel + 1;
-  if (npanel == a.n_panels) {
-    tile = tile_n;
-    npanel = 0;
-  }
-  if (tile >= a.n_tiles) return;
-  const int row0 = __ldg(a.tile_row0 + tile);
-  const unsigned bytes = (unsigned)(__ldg(a.tile_row0 + tile + 1) - row0) * 128u;
-  const unsigned at = (unsigned)tid * 2048u;
-  if (at < bytes)
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(
-                     a.X1 + npanel * panel_stride + (size_t)row0 * kTilePanel + at / 8),
-                 "r"(min(2048u, bytes - at))
-                 : "memory");
-}
-
 // THREADS = 512 with one CTA per SM for tiles that fill the shared memory, 256 with three CTAs
 // per SM (85 registers) for tiles of at most a third of it.
 // Same for a work item = (panel, tile) of the panel-major order of the row-record sweep.
@@ -394,9 +350,6 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
     __syncthreads();
 
     for (int panel = panel_of_work; panel == panel_of_work; ++panel) {
-#ifdef POLFED_TILED_PROFILE
-      long long t0 = clock64(), t1 = t0, t2 = t0, t3 = t0, t4 = t0;
-#endif
       const double* X1 = a.X1 + panel * panel_stride;
       const double* Pk = a.Pk + panel * panel_stride + (size_t)row0 * kTilePanel;
       const double* V = a.V + panel * panel_stride + (size_t)row0 * kTilePanel;
@@ -427,7 +380,6 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
         RowHead nx = load_head(rec, side, a.side_words, diag, base + slot, nrows, q);
         mbar_wait(&bar, parity);
         parity ^= 1u;
-        PROF_CLOCK(t1);
         for (; base < nrows; base = base_n, base_n = grab_chunk(chunk, lane)) {
           const int pos = base + slot;
           const bool active = pos < nrows;
@@ -441,17 +393,17 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
           d4_zero(g2);
           int dst = (int)hd.side.x;
           if (active) {
-            if (!PROF_SKIP(SKIP_PK)) pk = ldg256_stream(Pk + (size_t)pos * kTilePanel + 4 * q, pol_first);
+            pk = ldg256_stream(Pk + (size_t)pos * kTilePanel + 4 * q, pol_first);
             if (MODE == MODE_LAST) dst = __ldg(dst_map + pos);
           }
-          if (hd.side.y != kCrossNone && !PROF_SKIP(SKIP_CROSS))
+          if (hd.side.y != kCrossNone)
             g0 = ldg256(X1 + (size_t)(hd.side.y & kCrossPosMask) * kTilePanel + 4 * q);
-          if (hd.side.z != kCrossNone && !PROF_SKIP(SKIP_CROSS))
+          if (hd.side.z != kCrossNone)
             g1 = ldg256(X1 + (size_t)(hd.side.z & kCrossPosMask) * kTilePanel + 4 * q);
-          if (hd.side.w != kCrossNone && !PROF_SKIP(SKIP_CROSS))
+          if (hd.side.w != kCrossNone)
             g2 = ldg256(X1 + (size_t)(hd.side.w & kCrossPosMask) * kTilePanel + 4 * q);
           const int deg = __shfl_sync(0xffffffffu, (int)hd.rq.x, 0, 4);
-          const int max_deg = PROF_SKIP(SKIP_HOPS2) ? 0 : __reduce_max_sync(0xffffffffu, deg);
+          const int max_deg = __reduce_max_sync(0xffffffffu, deg);
           double2 acc_f = zero2, acc_s = zero2;
           tile_hops<NC>(hd.rq, max_deg, x_first, x_second, a.coef, acc_f, acc_s);
           if (active) {  // diagonal: own row of the shared tile
@@ -485,8 +437,8 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
             if (MODE == MODE_LAST) {
               stg256_hint(a.W + (size_t)dst * a.w_ld + panel * kTilePanel + 4 * q, b, pol_first);
             } else {
-              if (!PROF_SKIP(SKIP_BOUT)) stg256_hint(Bout + (size_t)dst * kTilePanel + 4 * q, b, pol_first);
-              if (!PROF_SKIP(SKIP_SCRATCH)) stg256_hint(scratch + (size_t)pos * kTilePanel + 4 * q, b, pol_last);
+              stg256_hint(Bout + (size_t)dst * kTilePanel + 4 * q, b, pol_first);
+              stg256_hint(scratch + (size_t)pos * kTilePanel + 4 * q, b, pol_last);
             }
           }
         }
@@ -500,7 +452,6 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
       __threadfence_block();
       fence_proxy_async();
       __syncthreads();
-      PROF_CLOCK(t2);
       if (tid == 0) {
         tile_load(smem_raw, scratch, (unsigned)nrows * 128u, &bar, pol_last);
         s_chunk[(phase + 1) & 1] = 0;
@@ -514,7 +465,6 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
         next_work_prefetch(a, s_tile[(it + 1) & 1], panel_stride, tid);
       mbar_wait(&bar, parity);
       parity ^= 1u;
-      PROF_CLOCK(t3);
       // the parked copy is dead once it is back in shared memory: drop it from L2 unwritten
       for (int r = tid; r < nrows; r += THREADS)
         asm volatile("discard.global.L2 [%0], 128;" ::"l"(scratch + (size_t)r * kTilePanel) : "memory");
@@ -535,11 +485,11 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
         int dst = 0;
         if (active) {
           dst = __ldg(dst_map + pos);
-          if (a.rs != 0.0 && !PROF_SKIP(SKIP_X1)) x1 = ldg256(X1 + ((size_t)row0 + pos) * kTilePanel + 4 * q);
-          if (a.cs != 0.0 && !PROF_SKIP(SKIP_V)) v = ldg256_stream(V + (size_t)pos * kTilePanel + 4 * q, pol_first);
+          if (a.rs != 0.0) x1 = ldg256(X1 + ((size_t)row0 + pos) * kTilePanel + 4 * q);
+          if (a.cs != 0.0) v = ldg256_stream(V + (size_t)pos * kTilePanel + 4 * q, pol_first);
         }
         const int deg = __shfl_sync(0xffffffffu, (int)rq.x, 0, 4);
-        const int max_deg = PROF_SKIP(SKIP_HOPS3) ? 0 : __reduce_max_sync(0xffffffffu, deg);
+        const int max_deg = __reduce_max_sync(0xffffffffu, deg);
         double2 acc_f = zero2, acc_s = zero2;
         tile_hops<NC>(rq, max_deg, x_first, x_second, a.coef, acc_f, acc_s);
         if (active) {
@@ -554,452 +504,8 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
           y.y = fma(a.cs, v.y, fma(a.rs, x1.y, y.y));
           y.z = fma(a.cs, v.z, fma(a.rs, x1.z, y.z));
           y.w = fma(a.cs, v.w, fma(a.rs, x1.w, y.w));
-          if (!PROF_SKIP(SKIP_POUT)) stg256_hint(Pout + (size_t)dst * kTilePanel + 4 * q, y, pol_first);
+          stg256_hint(Pout + (size_t)dst * kTilePanel + 4 * q, y, pol_first);
         }
-      }
-      __syncthreads();  // all reads of the tile done before the next bulk copy
-#ifdef POLFED_TILED_PROFILE
-      t4 = clock64();
-      if (tid == 0 && a.prof) {
-        unsigned long long* pr = a.prof + blockIdx.x * 8;
-        pr[0] += t1 - t0;
-        pr[1] += t2 - t1;
-        pr[2] += t3 - t2;
-        pr[3] += t4 - t3;
-        pr[4] += 1;
-        pr[5] += nrows;
-      }
-#endif
-    }
-  }
-}
-
-// ---- fibre mode (tiled.cuh): 8 lanes own a fibre of up to 10 rows ----------------------------
-
-__device__ __forceinline__ int grab_one(int* counter, int lane) {  // a warp claims one chunk
-  int v = 0;
-  if (lane == 0) v = atomicAdd(counter, 1);
-  return __shfl_sync(0xffffffffu, v, 0);
-}
-
-__device__ __forceinline__ double2 ldg128(const double* p) {
-  return __ldg(reinterpret_cast<const double2*>(p));
-}
-__device__ __forceinline__ double2 ldg128_stream(const double* p, uint64_t pol) {
-  double2 r;
-  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;"
-               : "=d"(r.x), "=d"(r.y)
-               : "l"(p), "l"(pol));
-  return r;
-}
-__device__ __forceinline__ void stg128_hint(double* p, const double2 r, uint64_t pol) {
-  asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p),
-               "d"(r.x), "d"(r.y), "l"(pol)
-               : "memory");
-}
-__device__ __forceinline__ void fma2(double c, const double2 x, double2& acc) {
-  acc.x = fma(c, x.x, acc.x);
-  acc.y = fma(c, x.y, acc.y);
-}
-
-// Per-row records of a fibre are loaded once per chunk, one row per lane (lane l8 holds rows l8
-// and l8 + 8), before the hops, and handed to the 8 lanes row by row with shuffles: no dependent
-// global load is left in the per-row tail.  R is a compile-time row number.
-template <int R>
-__device__ __forceinline__ uint32_t row_bcast(uint32_t a_word, uint32_t b_word) {
-  return __shfl_sync(0xffffffffu, R < 8 ? a_word : b_word, R & 7, 8);
-}
-
-// Header of a fibre record.
-struct FibreHead {
-  int pos0, rows, n_hops, dense_off;
-};
-__device__ __forceinline__ FibreHead fibre_head(uint32_t h, const SweepArgs& a) {
-  FibreHead f;
-  const int j = (h >> 11) & 7;
-  f.pos0 = h & 0x7ff;
-  f.n_hops = (h >> 14) & 15;
-  f.rows = ((h >> 18) & 1u) ? a.fibre_size[j] : 0;
-  f.dense_off = a.dense_off[j];
-  return f;
-}
-
-// acc[r] += (in-fibre hops + `self` x own row) for the rows of the fibre held in xo.
-__device__ __forceinline__ void fibre_dense(const SweepArgs& a, const FibreHead& f,
-                                            const double2 (&xo)[kFibreMaxRows],
-                                            double2 (&acc)[kFibreMaxRows]) {
-#pragma unroll
-  for (int r = 0; r < kFibreMaxRows; ++r) {
-    if (r >= f.rows) break;
-    const double* m = a.dense + f.dense_off + r * f.rows;
-#pragma unroll
-    for (int c = 0; c < kFibreMaxRows; ++c) {
-      if (c >= f.rows) break;
-      fma2(m[c], xo[c], acc[r]);
-    }
-  }
-}
-
-// Hops among the upper tile sites: one entry moves the whole fibre.  w_me is this lane's word of
-// the fibre record (lane l8 holds word l8); max_hops is warp-uniform.
-template <int NC>
-__device__ __forceinline__ void fibre_hops(const SweepArgs& a, const FibreHead& f, uint32_t w_me,
-                                           int max_hops, const unsigned char* __restrict__ xl,
-                                           double2 (&acc)[kFibreMaxRows]) {
-#pragma unroll
-  for (int w = 1; w < kFibreRecWords; ++w) {
-    if (2 * (w - 1) >= max_hops) break;
-    const uint32_t word = __shfl_sync(0xffffffffu, w_me, w, 8);
-    if (2 * (w - 1) < f.n_hops) {
-      const double cf = signed_coef(pick_coef<NC>(word & 3u, a.coef), word << 1);
-      const unsigned char* src = xl + (word & 0x3ff80u);
-#pragma unroll
-      for (int r = 0; r < kFibreMaxRows; ++r) {
-        if (r >= f.rows) break;
-        fma2(cf, *reinterpret_cast<const double2*>(src + r * 128), acc[r]);
-      }
-    }
-    if (2 * w - 1 < f.n_hops) {
-      const double cf = signed_coef(pick_coef<NC>((word >> 2) & 3u, a.coef), word);
-      const unsigned char* src = xl + ((word >> 11) & 0x3ff80u);
-#pragma unroll
-      for (int r = 0; r < kFibreMaxRows; ++r) {
-        if (r >= f.rows) break;
-        fma2(cf, *reinterpret_cast<const double2*>(src + r * 128), acc[r]);
-      }
-    }
-  }
-}
-
-// Hops between the low g sites and the rest: up to three neighbours of one row (row record rr).
-template <int NC>
-__device__ __forceinline__ void row_hops(const SweepArgs& a, const uint2 rr,
-                                         const unsigned char* __restrict__ xl, double2& acc) {
-  const uint32_t cnt = rr.x >> 28;
-  const uint32_t e[kFibreRowHops] = {rr.x & 0x3fffu, (rr.x >> 14) & 0x3fffu, rr.y & 0x3fffu};
-#pragma unroll
-  for (int i = 0; i < kFibreRowHops; ++i)
-    if ((uint32_t)i < cnt) {
-      const double cf = signed_coef(pick_coef<NC>((e[i] >> 11) & 3u, a.coef), e[i] << 18);
-      fma2(cf, *reinterpret_cast<const double2*>(xl + (e[i] & 0x7ffu) * 128u), acc);
-    }
-}
-
-template <int NC, int MODE, int THREADS>
-__global__ void __launch_bounds__(THREADS, THREADS == kTileThreads ? 1 : kTileSmallCtas)
-    tiled_fibre_kernel(const SweepArgs a) {
-  constexpr int kIterRows = (THREADS / 32) * kRowsPerIter;  // MODE_INIT's static loop
-  extern __shared__ __align__(128) unsigned char smem_raw[];  // the tile panel
-  __shared__ uint64_t bar;
-  __shared__ int s_tile[2];
-  __shared__ int s_chunk[2];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int grp = lane >> 3, l8 = lane & 7;       // fibre of the chunk, 16-byte slice of a row
-  const unsigned char* xl = smem_raw + 16 * l8;
-  if (tid == 0) {
-    mbar_init(&bar, 1);
-    s_tile[0] = atomicAdd(a.counter, 1);
-    s_chunk[0] = s_chunk[1] = 0;
-  }
-  __syncthreads();
-  unsigned parity = 0;
-  int phase = 0;
-  double* scratch = a.scratch + (size_t)blockIdx.x * a.max_tile_rows * kTilePanel;
-  const size_t panel_stride = (size_t)a.n * kTilePanel;
-  const uint64_t pol_first = l2_policy_evict_first(), pol_last = l2_policy_evict_last();
-  const double2 zero2 = make_double2(0.0, 0.0);
-
-  for (int it = 0;; ++it) {
-    const int tile = s_tile[it & 1];
-    if (tile >= a.n_tiles) break;
-    if (tid == 0) s_tile[(it + 1) & 1] = atomicAdd(a.counter, 1);
-    const int row0 = __ldg(a.tile_row0 + tile);
-    const int nrows = __ldg(a.tile_row0 + tile + 1) - row0;
-    const int n_chunks = __ldg(a.tile_chunks + tile);
-    const uint32_t* frec = a.fibre_rec + (size_t)__ldg(a.tile_fib0 + tile) * kFibreRecWords;
-    const uint2* rrec = reinterpret_cast<const uint2*>(a.row_rec) + __ldg(a.tile_rec0 + tile);
-    const uint32_t* side = a.side + (size_t)row0 * a.side_words;
-    const double* diag = a.diag + row0;
-    const int32_t* dst_map = a.dst_map + row0;
-    __syncthreads();
-
-    for (int panel = 0; panel < a.n_panels; ++panel) {
-      const double* X1 = a.X1 + panel * panel_stride;
-      const double* Pk = a.Pk + panel * panel_stride + (size_t)row0 * kTilePanel;
-      const double* V = a.V + panel * panel_stride + (size_t)row0 * kTilePanel;
-      double* Bout = a.Bout + panel * panel_stride;
-      double* Pout = a.Pout + panel * panel_stride;
-
-      if (MODE == MODE_INIT) {
-        // ---- b_K = c_K V: four lanes per row, 32 bytes each ---------------------------------
-        const int q = lane & 3;
-        for (int pos = warp * kRowsPerIter + (lane >> 2); pos < nrows; pos += kIterRows) {
-          const int dst = __ldg(dst_map + pos);
-          D4 b = ldg256_stream(V + (size_t)pos * kTilePanel + 4 * q, pol_first);
-          b.x *= a.cK;
-          b.y *= a.cK;
-          b.z *= a.cK;
-          b.w *= a.cK;
-          stg256_hint(Bout + (size_t)dst * kTilePanel + 4 * q, b, pol_first);
-          stg256_hint(scratch + (size_t)pos * kTilePanel + 4 * q, b, pol_last);
-        }
-      } else {
-        // ---- phase 2: b_k = P_k + p_k (O_l + DM) b_{k+1} ---------------------------------------
-        if (tid == 0) {
-          tile_load(smem_raw, X1 + (size_t)row0 * kTilePanel, (unsigned)nrows * 128u, &bar,
-                    pol_last);
-          s_chunk[(phase + 1) & 1] = 0;
-        }
-        int* const chunk = &s_chunk[phase & 1];
-        ++phase;
-        int c = grab_one(chunk, lane), c_n = grab_one(chunk, lane);
-        uint32_t w_n = c < n_chunks
-                           ? __ldg(frec + (size_t)(c * kFibresPerChunk + grp) * kFibreRecWords + l8)
-                           : 0u;
-        mbar_wait(&bar, parity);
-        parity ^= 1u;
-        for (; c < n_chunks; c = c_n, c_n = grab_one(chunk, lane)) {
-          const uint32_t w_me = w_n;
-          w_n = c_n < n_chunks
-                    ? __ldg(frec + (size_t)(c_n * kFibresPerChunk + grp) * kFibreRecWords + l8)
-                    : 0u;
-          const FibreHead f = fibre_head(__shfl_sync(0xffffffffu, w_me, 0, 8), a);
-          const int max_hops = __reduce_max_sync(0xffffffffu, f.n_hops);
-          const int max_rows = __reduce_max_sync(0xffffffffu, f.rows);
-          // per-row records, one row per lane
-          uint2 rrA = make_uint2(0u, 0u), rrB = rrA;
-          uint4 sdA = make_uint4(0u, kCrossNone, kCrossNone, kCrossNone), sdB = sdA;
-          uint32_t dnA = 0u, dnB = 0u;  // MODE_LAST: row in the caller's order
-          if (l8 < f.rows) {
-            rrA = __ldg(rrec + f.pos0 + l8);
-            sdA = __ldg(reinterpret_cast<const uint4*>(side + (size_t)(f.pos0 + l8) * a.side_words));
-            if (MODE == MODE_LAST) dnA = (uint32_t)__ldg(dst_map + f.pos0 + l8);
-          }
-          if (l8 + 8 < f.rows) {
-            rrB = __ldg(rrec + f.pos0 + l8 + 8);
-            sdB = __ldg(
-                reinterpret_cast<const uint4*>(side + (size_t)(f.pos0 + l8 + 8) * a.side_words));
-            if (MODE == MODE_LAST) dnB = (uint32_t)__ldg(dst_map + f.pos0 + l8 + 8);
-          }
-          double2 xo[kFibreMaxRows], acc[kFibreMaxRows];
-#pragma unroll
-          for (int r = 0; r < kFibreMaxRows; ++r) {
-            xo[r] = zero2;
-            acc[r] = zero2;
-            if (r < f.rows) {
-              xo[r] = *reinterpret_cast<const double2*>(xl + (size_t)(f.pos0 + r) * 128);
-              const double dg = __ldg(diag + f.pos0 + r);
-              acc[r].x = dg * xo[r].x;
-              acc[r].y = dg * xo[r].y;
-            }
-          }
-          fibre_dense(a, f, xo, acc);
-          // the rows' share of P_k replaces the own rows in the registers and flies during the hops
-#pragma unroll
-          for (int r = 0; r < kFibreMaxRows; ++r)
-            if (r < f.rows)
-              xo[r] = ldg128_stream(Pk + (size_t)(f.pos0 + r) * kTilePanel + 2 * l8, pol_first);
-          fibre_hops<NC>(a, f, w_me, max_hops, xl, acc);
-          {  // b_k = P_k + p (...) = p (acc + P_k / p): P_k leaves the registers before the tail
-            const double inv_pf = 1.0 / a.pf;
-#pragma unroll
-            for (int r = 0; r < kFibreMaxRows; ++r) fma2(inv_pf, xo[r], acc[r]);
-          }
-          // per-row tail, two rows in flight: records of row r + 1 are handed out and its cross-cut
-          // rows requested while row r is finished
-          uint4 sd_c;
-          uint2 rr_c;
-          uint32_t dn_c = 0u;
-          double2 g_c[3];
-          auto fetch = [&](auto R, uint4& sd, uint2& rr, uint32_t& dn, double2 (&g)[3]) {
-            constexpr int RR = decltype(R)::value;
-            sd.x = row_bcast<RR>(sdA.x, sdB.x);
-            sd.y = row_bcast<RR>(sdA.y, sdB.y);
-            sd.z = row_bcast<RR>(sdA.z, sdB.z);
-            sd.w = row_bcast<RR>(sdA.w, sdB.w);
-            rr.x = row_bcast<RR>(rrA.x, rrB.x);
-            rr.y = row_bcast<RR>(rrA.y, rrB.y);
-            if (MODE == MODE_LAST) dn = row_bcast<RR>(dnA, dnB);
-            const uint32_t cw[3] = {sd.y, sd.z, sd.w};
-#pragma unroll
-            for (int j = 0; j < 3; ++j) {
-              g[j] = zero2;
-              if (cw[j] != kCrossNone)
-                g[j] = ldg128(X1 + (size_t)(cw[j] & kCrossPosMask) * kTilePanel + 2 * l8);
-            }
-          };
-          auto finish = [&](int r, const uint4& sd, const uint2& rr, uint32_t dn,
-                            const double2 (&g)[3], double2& ac) {
-            if (r >= f.rows) return;
-            const int pos = f.pos0 + r;
-            row_hops<NC>(a, rr, xl, ac);
-            fma2(signed_coef(a.ccoef[(sd.y >> kCrossPosBits) & 15u], sd.y), g[0], ac);
-            fma2(signed_coef(a.ccoef[(sd.z >> kCrossPosBits) & 15u], sd.z), g[1], ac);
-            fma2(signed_coef(a.ccoef[(sd.w >> kCrossPosBits) & 15u], sd.w), g[2], ac);
-            if (a.side_words > 4) {  // cross-cut words 3..6 (wide cuts only)
-              const uint4 more =
-                  __ldg(reinterpret_cast<const uint4*>(side + (size_t)pos * 8 + 4));
-              const uint32_t cw[4] = {more.x, more.y, more.z, more.w};
-#pragma unroll
-              for (int j = 0; j < 4; ++j)
-                if (cw[j] != kCrossNone)
-                  fma2(signed_coef(a.ccoef[(cw[j] >> kCrossPosBits) & 15u], cw[j]),
-                       ldg128(X1 + (size_t)(cw[j] & kCrossPosMask) * kTilePanel + 2 * l8), ac);
-            }
-            double2 b;
-            b.x = a.pf * ac.x;
-            b.y = a.pf * ac.y;
-            if (MODE == MODE_LAST) {
-              stg128_hint(a.W + (size_t)dn * a.w_ld + panel * kTilePanel + 2 * l8, b, pol_first);
-            } else {
-              stg128_hint(Bout + (size_t)sd.x * kTilePanel + 2 * l8, b, pol_first);
-              stg128_hint(scratch + (size_t)pos * kTilePanel + 2 * l8, b, pol_last);
-            }
-          };
-          fetch(std::integral_constant<int, 0>{}, sd_c, rr_c, dn_c, g_c);
-#define POLFED_FIBRE_ROW(R)                                                              \
-  if (R < max_rows) {                                                                    \
-    uint4 sd_n = make_uint4(0u, kCrossNone, kCrossNone, kCrossNone);                     \
-    uint2 rr_n = make_uint2(0u, 0u);                                                     \
-    uint32_t dn_n = 0u;                                                                  \
-    double2 g_n[3] = {zero2, zero2, zero2};                                              \
-    if (R + 1 < max_rows)                                                                \
-      fetch(std::integral_constant<int, (R + 1 < kFibreMaxRows ? R + 1 : 0)>{}, sd_n, rr_n, dn_n, \
-            g_n);                                                                        \
-    finish(R, sd_c, rr_c, dn_c, g_c, acc[R]);                                            \
-    sd_c = sd_n;                                                                         \
-    rr_c = rr_n;                                                                         \
-    dn_c = dn_n;                                                                         \
-    g_c[0] = g_n[0];                                                                     \
-    g_c[1] = g_n[1];                                                                     \
-    g_c[2] = g_n[2];                                                                     \
-  }
-          POLFED_FIBRE_ROW(0)
-          POLFED_FIBRE_ROW(1)
-          POLFED_FIBRE_ROW(2)
-          POLFED_FIBRE_ROW(3)
-          POLFED_FIBRE_ROW(4)
-          POLFED_FIBRE_ROW(5)
-          POLFED_FIBRE_ROW(6)
-          POLFED_FIBRE_ROW(7)
-          POLFED_FIBRE_ROW(8)
-          POLFED_FIBRE_ROW(9)
-#undef POLFED_FIBRE_ROW
-        }
-      }
-      if (MODE == MODE_LAST) {
-        __syncthreads();  // the next bulk copy overwrites the tile
-        continue;
-      }
-
-      // ---- b_k becomes the shared tile ------------------------------------------------------
-      __threadfence_block();
-      fence_proxy_async();
-      __syncthreads();
-      if (tid == 0) {
-        tile_load(smem_raw, scratch, (unsigned)nrows * 128u, &bar, pol_last);
-        s_chunk[(phase + 1) & 1] = 0;
-      }
-      int* const chunk = &s_chunk[phase & 1];
-      ++phase;
-      int c = grab_one(chunk, lane), c_n = grab_one(chunk, lane);
-      uint32_t w_n = c < n_chunks
-                         ? __ldg(frec + (size_t)(c * kFibresPerChunk + grp) * kFibreRecWords + l8)
-                         : 0u;
-      if (MODE == MODE_STEP)
-        next_tile_prefetch(a, tile, s_tile[(it + 1) & 1], panel, panel_stride, tid);
-      mbar_wait(&bar, parity);
-      parity ^= 1u;
-      // the parked copy is dead once it is back in shared memory: drop it from L2 unwritten
-      for (int r = tid; r < nrows; r += THREADS)
-        asm volatile("discard.global.L2 [%0], 128;" ::"l"(scratch + (size_t)r * kTilePanel) : "memory");
-
-      // ---- phase 3: P_{k-1} = c_{k-1} V + p_{k-1} O_l b_k + q_{k-1} b_k + r b_{k+1} ------------
-      const double q_over_p = a.qs / a.ps;
-      for (; c < n_chunks; c = c_n, c_n = grab_one(chunk, lane)) {
-        const uint32_t w_me = w_n;
-        w_n = c_n < n_chunks
-                  ? __ldg(frec + (size_t)(c_n * kFibresPerChunk + grp) * kFibreRecWords + l8)
-                  : 0u;
-        const FibreHead f = fibre_head(__shfl_sync(0xffffffffu, w_me, 0, 8), a);
-        const int max_hops = __reduce_max_sync(0xffffffffu, f.n_hops);
-        const int max_rows = __reduce_max_sync(0xffffffffu, f.rows);
-        uint2 rrA = make_uint2(0u, 0u), rrB = rrA;
-        uint32_t dnA = 0u, dnB = 0u;  // position in the other layout
-        if (l8 < f.rows) {
-          rrA = __ldg(rrec + f.pos0 + l8);
-          dnA = (uint32_t)__ldg(dst_map + f.pos0 + l8);
-        }
-        if (l8 + 8 < f.rows) {
-          rrB = __ldg(rrec + f.pos0 + l8 + 8);
-          dnB = (uint32_t)__ldg(dst_map + f.pos0 + l8 + 8);
-        }
-        double2 xo[kFibreMaxRows], acc[kFibreMaxRows];
-#pragma unroll
-        for (int r = 0; r < kFibreMaxRows; ++r) {
-          xo[r] = zero2;
-          acc[r] = zero2;
-          if (r < f.rows) {
-            xo[r] = *reinterpret_cast<const double2*>(xl + (size_t)(f.pos0 + r) * 128);
-            acc[r].x = q_over_p * xo[r].x;  // q b_k, scaled by p with the hops below
-            acc[r].y = q_over_p * xo[r].y;
-          }
-        }
-        fibre_dense(a, f, xo, acc);
-#pragma unroll
-        for (int r = 0; r < kFibreMaxRows; ++r) {  // c V of the rows flies during the hops
-          xo[r] = zero2;
-          if (r < f.rows && a.cs != 0.0)
-            xo[r] = ldg128_stream(V + (size_t)(f.pos0 + r) * kTilePanel + 2 * l8, pol_first);
-        }
-        fibre_hops<NC>(a, f, w_me, max_hops, xl, acc);
-        {  // c V folded into the sum that p scales: V leaves the registers before the tail
-          const double c_over_p = a.cs / a.ps;
-#pragma unroll
-          for (int r = 0; r < kFibreMaxRows; ++r) fma2(c_over_p, xo[r], acc[r]);
-        }
-        uint2 rr_c;
-        uint32_t dn_c;
-        double2 x1_c;
-        auto fetch = [&](auto R, uint2& rr, uint32_t& dn, double2& x1) {
-          constexpr int RR = decltype(R)::value;
-          rr.x = row_bcast<RR>(rrA.x, rrB.x);
-          rr.y = row_bcast<RR>(rrA.y, rrB.y);
-          dn = row_bcast<RR>(dnA, dnB);
-          x1 = zero2;
-          if (RR < f.rows && a.rs != 0.0)
-            x1 = ldg128(X1 + ((size_t)row0 + f.pos0 + RR) * kTilePanel + 2 * l8);
-        };
-        fetch(std::integral_constant<int, 0>{}, rr_c, dn_c, x1_c);
-#define POLFED_FIBRE_ROW(R)                                                                    \
-  if (R < max_rows) {                                                                          \
-    uint2 rr_n = make_uint2(0u, 0u);                                                           \
-    uint32_t dn_n = 0u;                                                                        \
-    double2 x1_n = zero2;                                                                      \
-    if (R + 1 < max_rows)                                                                      \
-      fetch(std::integral_constant<int, (R + 1 < kFibreMaxRows ? R + 1 : 0)>{}, rr_n, dn_n, x1_n); \
-    if (R < f.rows) {                                                                          \
-      row_hops<NC>(a, rr_c, xl, acc[R]);                                                       \
-      double2 y;                                                                               \
-      y.x = fma(a.rs, x1_c.x, a.ps * acc[R].x);                                                \
-      y.y = fma(a.rs, x1_c.y, a.ps * acc[R].y);                                                \
-      stg128_hint(Pout + (size_t)dn_c * kTilePanel + 2 * l8, y, pol_first);                    \
-    }                                                                                          \
-    rr_c = rr_n;                                                                               \
-    dn_c = dn_n;                                                                               \
-    x1_c = x1_n;                                                                               \
-  }
-        POLFED_FIBRE_ROW(0)
-        POLFED_FIBRE_ROW(1)
-        POLFED_FIBRE_ROW(2)
-        POLFED_FIBRE_ROW(3)
-        POLFED_FIBRE_ROW(4)
-        POLFED_FIBRE_ROW(5)
-        POLFED_FIBRE_ROW(6)
-        POLFED_FIBRE_ROW(7)
-        POLFED_FIBRE_ROW(8)
-        POLFED_FIBRE_ROW(9)
-#undef POLFED_FIBRE_ROW
       }
       __syncthreads();  // all reads of the tile done before the next bulk copy
     }
@@ -1036,21 +542,8 @@ int launch_sweep_t(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
   return POLFED_OK;
 }
 
-template <int NC, int THREADS>
-int launch_fibre_t(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
-  if (a.mode == MODE_INIT)
-    tiled_fibre_kernel<NC, MODE_INIT, THREADS><<<p->grid, THREADS, p->smem_bytes, st>>>(a);
-  else if (a.mode == MODE_LAST)
-    tiled_fibre_kernel<NC, MODE_LAST, THREADS><<<p->grid, THREADS, p->smem_bytes, st>>>(a);
-  else
-    tiled_fibre_kernel<NC, MODE_STEP, THREADS><<<p->grid, THREADS, p->smem_bytes, st>>>(a);
-  POLFED_LAUNCH_CHECK("tiled_fibre_kernel");
-  return POLFED_OK;
-}
-
 template <int NC>
 int launch_sweep(const TiledPlan* p, const SweepArgs& a, cudaStream_t st) {
-  if (p->fibre_g) return launch_fibre_t<NC, kTileThreads>(p, a, st);
   return p->threads == kTileThreads ? launch_sweep_t<NC, kTileThreads>(p, a, st)
                                     : launch_sweep_t<NC, kTileSmallThreads>(p, a, st);
 }
@@ -1064,18 +557,7 @@ int sweep(const TiledPlan* p, int layout, SweepArgs a, cudaStream_t st) {
   for (int c = 0; c <= kTileMaxCrossCoef; ++c) a.ccoef[c] = L.ccoef[c];
   a.dst_map = (a.mode == MODE_LAST) ? L.d_to_natural : L.d_to_other;
   for (int c = 0; c < kTileMaxCoef; ++c) a.coef[c] = L.coef[c];
-  if (p->fibre_g) {
-    a.fibre_rec = L.d_fibre_rec;
-    a.row_rec = L.d_row_rec;
-    a.tile_fib0 = p->d_tile_fib0;
-    a.tile_chunks = p->d_tile_chunks;
-    for (int j = 0; j <= kFibreMaxSites; ++j) {
-      a.fibre_size[j] = p->fibre_size[j];
-      a.dense_off[j] = p->dense_off[j];
-    }
-    for (int i = 0; i < kFibreDense; ++i) a.dense[i] = L.dense[i];
-  }
-  POLFED_CUDA(cudaMemsetAsync(p->d_counter, 0, sizeof(int), st));
+  POLFED_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(int), st));
   return L.n_coef <= 2 ? launch_sweep<2>(p, a, st) : launch_sweep<4>(p, a, st);
 }
 
@@ -1104,31 +586,6 @@ int configure_all(TiledPlan* p, int* occ) {
   return POLFED_OK;
 }
 
-template <int NC, int MODE, int THREADS>
-int configure_fibre_one(TiledPlan* p, int* occ) {
-  POLFED_CUDA(cudaFuncSetAttribute(tiled_fibre_kernel<NC, MODE, THREADS>,
-                                   cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)p->smem_bytes));
-  int o = 0;
-  POLFED_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-      &o, tiled_fibre_kernel<NC, MODE, THREADS>, THREADS, p->smem_bytes));
-  if (o < 1) return fail(POLFED_ECUDA, "tiled format: fibre kernel does not fit an SM");
-  *occ = (*occ == 0 || o < *occ) ? o : *occ;
-  return POLFED_OK;
-}
-
-template <int THREADS>
-int configure_fibre_all(TiledPlan* p, int* occ) {
-  int rc;
-  if ((rc = configure_fibre_one<2, MODE_STEP, THREADS>(p, occ))) return rc;
-  if ((rc = configure_fibre_one<2, MODE_INIT, THREADS>(p, occ))) return rc;
-  if ((rc = configure_fibre_one<2, MODE_LAST, THREADS>(p, occ))) return rc;
-  if ((rc = configure_fibre_one<4, MODE_STEP, THREADS>(p, occ))) return rc;
-  if ((rc = configure_fibre_one<4, MODE_INIT, THREADS>(p, occ))) return rc;
-  if ((rc = configure_fibre_one<4, MODE_LAST, THREADS>(p, occ))) return rc;
-  return POLFED_OK;
-}
-
 }  // namespace
 
 int tiled_configure_launch(TiledPlan* p) {
@@ -1137,10 +594,7 @@ int tiled_configure_launch(TiledPlan* p) {
   // small tiles: several CTAs per SM hide each other's bulk-copy waits and barriers
   p->threads = (p->smem_bytes + 1024) * kTileSmallCtas <= 227u * 1024u ? kTileSmallThreads
                                                                         : kTileThreads;
-  if (p->fibre_g) p->threads = kTileThreads;  // the fibre kernel needs the registers of one CTA per SM
-  if (p->fibre_g) {
-    if ((rc = configure_fibre_all<kTileThreads>(p, &occ))) return rc;
-  } else if (p->threads == kTileThreads) {
+  if (p->threads == kTileThreads) {
     if ((rc = configure_all<kTileThreads>(p, &occ))) return rc;
   } else {
     if ((rc = configure_all<kTileSmallThreads>(p, &occ))) return rc;
@@ -1158,16 +612,22 @@ bool tiled_supports(const polfed_ham* ham, int s) {
   return ham && ham->tiled && (s == 16 || s == 32) && ham->n > 0;
 }
 
-// X/P pairs (4 blocks) + V in both layouts (2 blocks) + the per-CTA scratch
+size_t sector_workspace_bytes(const polfed_ham* ham, int s);  // sector_sweep.cu
+int sector_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* c, int s,
+                        const double* d_V, double* d_W, void* d_work, cudaStream_t st);
+
+// X/P pairs (4 blocks) + V in both layouts (2 blocks) + the per-CTA scratch + the tile counter
 size_t tiled_workspace_bytes(const polfed_ham* ham, int s) {
   const TiledPlan* p = ham->tiled;
+  if (p->sector) return sector_workspace_bytes(ham, s);
   return (size_t)6 * (size_t)ham->n * s * sizeof(double) +
-         (size_t)p->grid * p->max_tile_rows * 128;
+         (size_t)p->grid * p->max_tile_rows * 128 + 128;
 }
 
 int tiled_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const double* c,
                        int s, const double* d_V, double* d_W, void* d_work, cudaStream_t st) {
   const TiledPlan* p = ham->tiled;
+  if (p->sector) return sector_filter_apply(ham, a_, b_, K, c, s, d_V, d_W, d_work, st);
   const size_t len = (size_t)ham->n * s;
   double* base = static_cast<double*>(d_work);
   double* X[2] = {base, base + 2 * len};
@@ -1182,16 +642,6 @@ int tiled_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
   POLFED_LAUNCH_CHECK("tiled_pack_kernel");
 
   SweepArgs a{};
-#ifdef POLFED_TILED_PROFILE
-  static unsigned long long* d_prof = nullptr;
-  {
-    const char* e = getenv("POLFED_TILED_SKIP");
-    a.skip = e ? atoi(e) : 0;
-    if (!d_prof) POLFED_CUDA(cudaMalloc(&d_prof, sizeof(unsigned long long) * 8 * 1024));
-    POLFED_CUDA(cudaMemsetAsync(d_prof, 0, sizeof(unsigned long long) * 8 * 1024, st));
-    a.prof = d_prof;
-  }
-#endif
   a.n = ham->n;
   a.n_tiles = p->n_tiles;
   a.n_panels = n_panels;
@@ -1199,7 +649,8 @@ int tiled_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
   a.tile_row0 = p->d_tile_row0;
   a.tile_rec0 = p->d_tile_rec0;
   a.scratch = scratch;
-  a.counter = p->d_counter;
+  // the tile counter lives in the caller's workspace, so the handle stays read-only
+  a.counter = reinterpret_cast<int*>(scratch + (size_t)p->grid * p->max_tile_rows * kTilePanel);
   a.W = d_W;
   a.w_ld = s;
   auto pk = [&](int k) { return (k == 0 ? 1.0 : 2.0) / b_; };
@@ -1226,20 +677,6 @@ int tiled_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
     int rc = sweep(p, layout, a, st);
     if (rc) return rc;
   }
-#ifdef POLFED_TILED_PROFILE
-  {
-    static unsigned long long h[8 * 1024];
-    POLFED_CUDA(cudaStreamSynchronize(st));
-    POLFED_CUDA(cudaMemcpy(h, d_prof, sizeof(h), cudaMemcpyDeviceToHost));
-    double t[6] = {0, 0, 0, 0, 0, 0};
-    for (int b = 0; b < p->grid && b < 1024; ++b)
-      for (int i = 0; i < 6; ++i) t[i] += (double)h[b * 8 + i];
-    fprintf(stderr,
-            "tiled profile: skip=%d K=%d tile-panels=%.0f rows/tile-panel=%.1f cycles/tile-panel: "
-            "load %.0f phase2 %.0f reload %.0f phase3 %.0f\n",
-            a.skip, K, t[4], t[5] / t[4], t[0] / t[4], t[1] / t[4], t[2] / t[4], t[3] / t[4]);
-  }
-#endif
   return POLFED_OK;
 }
 

@@ -210,47 +210,3 @@ def test_tiled_full_size_config5_sampled_rows(P):
     P.polfed_fused_step(ham, s, 1.0 / b, -a / b, -1.0, c[0], B1, B2, V, B2)          # W
     diff = float((B2 - W).norm() / W.norm())
     assert diff <= 1e-13
-
-
-# ---- the experimental fibre mode of the tiled format (POLFED_TILED_FIBRE=1 at build time) --------
-
-@pytest.fixture
-def fibre_mode(monkeypatch):
-    monkeypatch.setenv("POLFED_TILED_FIBRE", "1")
-
-
-@pytest.mark.parametrize("K", [1, 2, 5, 40])
-@pytest.mark.parametrize("s", (16, 32))
-@pytest.mark.parametrize("L,n_up", [(8, 4), (12, 3), (13, 6), (14, 9), (16, 8)])
-def test_tiled_fibre_mode_random_coefficients(P, fibre_mode, L, n_up, s, K):
-    rng = np.random.default_rng(100 * L + n_up)
-    terms = workloads.fermion_terms(L, 1.0, 0.5, 1.0, rng.uniform(-2, 2, L))
-    H = core.build_csr(core.basis_states(L, n_up), terms)
-    V = workloads.start_block(H.n, s, seed=7 * L + K)
-    a, b = 0.37, 1.05 * gershgorin(H)
-    coeffs = np.random.default_rng(K).standard_normal(K + 1)
-    want = core.clenshaw(H, a, b, coeffs, V)
-    got = tiled_filter(P, build(P, L, n_up, terms), a, b, coeffs, V)
-    assert rel_l2(got, want) <= 1e-12
-
-
-def test_tiled_fibre_mode_signs_long_hops_and_xxz(P, fibre_mode):
-    L, n_up, s = 12, 5, 16
-    terms = [("HOPJW", 0, 1, -0.7), ("HOPJW", 1, 3, 0.7), ("EXCH", 2, 5, 0.3), ("HOPJW", 4, 0, 1.1),
-             ("EXCH", 1, 2, 0.25), ("HOPJW", 0, 1, 0.7),
-             ("HOPJW", 5, 6, 0.9), ("HOPJW", 3, 9, -0.4), ("EXCH", 11, 0, 0.6),
-             ("HOPJW", 7, 10, 0.8), ("EXCH", 6, 11, -0.8), ("HOPJW", 8, 9, 0.2),
-             ("NN", 2, 7, 0.5), ("N", 11, 11, -1.5), ("ZZ", 0, 6, 0.9), ("Z", 3, 3, 0.4)]
-    H = core.build_csr(core.basis_states(L, n_up), terms)
-    V = workloads.start_block(H.n, s, seed=5)
-    coeffs = np.random.default_rng(1).standard_normal(12)
-    a, b = -0.2, 1.1 * gershgorin(H)
-    got = tiled_filter(P, build(P, L, n_up, terms), a, b, coeffs, V)
-    assert rel_l2(got, core.clenshaw(H, a, b, coeffs, V)) <= 1e-12
-    w = workloads.make_workload(3, L_override=14)               # periodic XXZ
-    _, H = core.hamiltonian(w)
-    V = workloads.start_block(H.n, w.s, seed=2003)
-    coeffs = cheb.filter_coeffs(0.0, 300)
-    a, b = 0.1, 1.05 * gershgorin(H)
-    got = tiled_filter(P, build(P, w.n_sites, w.n_up, w.terms), a, b, coeffs, V)
-    assert rel_l2(got, core.clenshaw(H, a, b, coeffs, V)) <= 1e-9
