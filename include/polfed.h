@@ -101,7 +101,8 @@ enum {
   POLFED_FORMAT_CSR = 0,
   POLFED_FORMAT_SELL = 1,  /* CSR plus SELL-8-sigma, see below */
   POLFED_FORMAT_TILED = 2, /* CSR plus the tiled structured format below */
-  POLFED_FORMAT_FLIP = 3   /* CSR plus the matrix-free flip format below */
+  POLFED_FORMAT_FLIP = 3,  /* CSR plus the matrix-free flip format below */
+  POLFED_FORMAT_SECTOR = 4 /* the tiled format with register-resident tile-local hops, below */
 };
 
 /* Assemble H on the device as CSR: row_ptr int32[N+1], col int32[nnz] ascending within a

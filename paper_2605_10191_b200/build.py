@@ -66,7 +66,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     todo = [s for s in sources() if force or _obj_stale(s)]
 
     def compile_one(src: str) -> None:
-        cmd = [nvcc, *NVCC_FLAGS, "-I", os.path.join(ROOT, "include"), "-I", CSRC,
+        # POLFED_NVCC_EXTRA: extra nvcc flags for developer builds (e.g. a -D switch)
+        extra = os.environ.get("POLFED_NVCC_EXTRA", "").split()
+        cmd = [nvcc, *NVCC_FLAGS, *extra, "-I", os.path.join(ROOT, "include"), "-I", CSRC,
                "-c", src, "-o", _obj(src)]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")

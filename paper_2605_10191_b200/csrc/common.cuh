@@ -58,8 +58,8 @@ int assemble_csr(const polfed_basis* basis, const std::vector<DevTerm>& terms, i
                  const double* h_dot, cudaStream_t st, int32_t** out_row_ptr, int32_t** out_col,
                  double** out_val, long long* out_nnz);
 // tiled_plan.cu / tiled_sweep.cu: the tiled (matrix-free inside a tile) format, see tiled.cuh.
-int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& terms, cudaStream_t st,
-                     TiledPlan** out);
+int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& terms, bool sector,
+                     cudaStream_t st, TiledPlan** out);
 void destroy_tiled_plan(TiledPlan* plan);
 bool tiled_supports(const polfed_ham* ham, int s);
 size_t tiled_workspace_bytes(const polfed_ham* ham, int s);

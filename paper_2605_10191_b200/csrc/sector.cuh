@@ -22,7 +22,7 @@ namespace polfed {
 
 constexpr int kSecPanel = 8;       // columns per panel: 64-byte rows
 constexpr int kSecMaxG = 7;        // sites per group (C(7,3) = 35 rows of a fibre in registers)
-constexpr int kSecThreads = 384;
+constexpr int kSecThreads = 512;
 constexpr int kSecMaxUnits = 48;   // work units per class and view
 constexpr int kSecGroups = 4;      // lane groups (fibres) per warp: 8 lanes x 8 bytes per row
 

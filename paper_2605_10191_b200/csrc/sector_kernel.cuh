@@ -300,17 +300,16 @@ __device__ __forceinline__ int claim(int* counter, int step, int lane) {
   return __shfl_sync(0xffffffffu, v, 0);
 }
 
-// The structured part of one phase: dst = alpha O_l src + beta src (+ gamma dst), O_l = O_G1 + O_G2.
-// All warps of the CTA; one CTA barrier between the two views.
-template <int G1, int G2, bool NNN, bool JW>
-__device__ __forceinline__ void structured_pass(const SecArgs& a, int k, const uint16_t* units1,
-                                                const uint16_t* units2, int* ctr1, int* ctr2,
-                                                uint32_t src, uint32_t dst, double alpha, double beta,
-                                                double gamma, bool use_old, uint32_t& epoch, int lane) {
+// The structured part of one phase: dst = alpha O_l src + beta src (+ gamma dst), O_l = O_G1 + O_G2,
+// in two steps (all warps of the CTA), each followed by a CTA barrier.
+template <int G1, bool NNN, bool JW>
+__device__ __forceinline__ void structured_v1(const SecArgs& a, int k, const uint16_t* units1, int* ctr,
+                                              uint32_t src, uint32_t dst, double alpha, double beta,
+                                              double gamma, bool use_old, uint32_t& epoch, int lane) {
   const int grp = lane >> 3;
   const double at1 = alpha * a.t1, at2 = alpha * a.t2;
-  const int nu1 = a.tab.n_units[0][k], nu2 = a.tab.n_units[1][k];
-  for (int u = claim(ctr1, 1, lane); u < nu1; u = claim(ctr1, 1, lane)) {
+  const int nu1 = a.tab.n_units[0][k];
+  for (int u = claim(ctr, 1, lane); u < nu1; u = claim(ctr, 1, lane)) {
     const int unit = __ldg(units1 + u), j1 = unit & 7, i2 = (unit >> 3) * kSecGroups + grp;
     if (i2 < a.tab.n2[k - j1]) {
       const uint32_t off = (uint32_t)(a.tab.srow[k][j1] + i2 * a.tab.n1p[j1]) * 64u;
@@ -320,7 +319,15 @@ __device__ __forceinline__ void structured_pass(const SecArgs& a, int k, const u
   }
   __syncthreads();
   ++epoch;
-  for (int u = claim(ctr2, 1, lane); u < nu2; u = claim(ctr2, 1, lane)) {
+}
+template <int G2, bool NNN, bool JW>
+__device__ __forceinline__ void structured_v2(const SecArgs& a, int k, const uint16_t* units2, int* ctr,
+                                              uint32_t src, uint32_t dst, double alpha,
+                                              uint32_t& epoch, int lane) {
+  const int grp = lane >> 3;
+  const double at1 = alpha * a.t1, at2 = alpha * a.t2;
+  const int nu2 = a.tab.n_units[1][k];
+  for (int u = claim(ctr, 1, lane); u < nu2; u = claim(ctr, 1, lane)) {
     const int unit = __ldg(units2 + u), j1 = unit & 7, i1 = (unit >> 3) * kSecGroups + grp;
     if (i1 < a.tab.n1[j1]) {
       const uint32_t off = (uint32_t)(a.tab.srow[k][j1] + i1) * 64u;
@@ -349,6 +356,25 @@ __device__ __forceinline__ RowMeta load_meta(const uint4* meta, int pos, int nro
   return r;
 }
 
+// The global operands of a row of the phase-2 row pass: its cross-cut partners.
+struct RowOperands {
+  double2 h0, h1, h2;
+};
+__device__ __forceinline__ double2 load_stream_if(const double* rows, int pos, int nrows, bool on,
+                                                  uint64_t pol) {
+  double2 v = make_double2(0.0, 0.0);
+  if (on && pos < nrows) v = ldg128_stream(rows + (size_t)pos * kSecPanel, pol);
+  return v;
+}
+__device__ __forceinline__ RowOperands load_operands(const RowMeta& m, const double* X1) {
+  RowOperands o;
+  const uint32_t c0 = m.m0.w, c1 = m.m1.x, c2 = m.m1.y;
+  o.h0 = ldg128_l2_if(X1 + (size_t)(c0 & kPosMask) * kSecPanel, c0 != kCrossNone);
+  o.h1 = ldg128_l2_if(X1 + (size_t)(c1 & kPosMask) * kSecPanel, c1 != kCrossNone);
+  o.h2 = ldg128_l2_if(X1 + (size_t)(c2 & kPosMask) * kSecPanel, c2 != kCrossNone);
+  return o;
+}
+
 // Cross-group partners of a row: entry slots 0..2 carry t1, t2, t2 (sector.cuh).
 __device__ __forceinline__ void cross_group(const RowMeta& m, uint32_t s_tile, double t1, double t2,
                                             uint32_t epoch, double2& acc) {
@@ -361,21 +387,44 @@ __device__ __forceinline__ void cross_group(const RowMeta& m, uint32_t s_tile, d
   fma2(signed_coef(t2, e2 << 18), g2, acc);
 }
 
+// Ask L2 for `bytes` (a multiple of 16) at p, 2 KB per participating thread starting at thread t0.
+__device__ __forceinline__ void l2_prefetch(const void* p, unsigned bytes, int tid, int t0) {
+  const unsigned at = (unsigned)(tid - t0) * 2048u;
+  if (tid >= t0 && at < bytes)
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(static_cast<const char*>(p) + at),
+                 "r"(min(2048u, bytes - at))
+                 : "memory");
+}
+
 constexpr int kTailRows = 8;  // rows per warp iteration of the row passes: 4 lanes x 16 bytes each
+constexpr int kSecWarps = kSecThreads / 32;
+// Row passes: register sets, look-ahead of the row records and of the cross-cut operands.
+constexpr int kD = 6, kDM = 5, kDO = 2;
 
 template <int M, bool NNN, bool JW, int MODE>
 __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecArgs a) {
   constexpr int G1 = M / 2, G2 = M - G1;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ uint64_t bar;
-  __shared__ int s_work[2];
-  __shared__ int s_ctr[6];
-  const int tid = threadIdx.x, lane = tid & 31;
-  const int l8 = lane & 7;              // structured passes: 8 lanes x 8 bytes per row
+  __shared__ int4 s_work[2];  // work item, first row, rows, class of the tile
+  __shared__ int s_ctr[4];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int l8 = lane & 7;                   // structured passes: 8 lanes x 8 bytes per row
   const int q = lane & 3, slot = lane >> 2;  // row passes: 4 lanes x 16 bytes per row
+  const int total = a.n_tiles * a.n_panels;
+  auto next_work = [&]() {  // one thread: claim a work item and look its tile up
+    int4 w = make_int4(atomicAdd(a.counter, 1), 0, 0, 0);
+    if (w.x < total) {
+      const int tile = w.x % a.n_tiles;
+      w.y = __ldg(a.tile_row0 + tile);
+      w.z = __ldg(a.tile_row0 + tile + 1) - w.y;
+      w.w = __ldg(a.tile_class + tile);
+    }
+    return w;
+  };
   if (tid == 0) {
     mbar_init(&bar, 1);
-    s_work[0] = atomicAdd(a.counter, 1);
+    s_work[0] = next_work();
   }
   __syncthreads();
   unsigned parity = 0;
@@ -383,136 +432,167 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
   const size_t panel_stride = (size_t)a.n * kSecPanel;
   const uint64_t pol_first = policy_evict_first(), pol_last = policy_evict_last();
   const uint32_t sA = smem_u32(smem_raw), sB = sA + a.buf_bytes;
-  const int total = a.n_tiles * a.n_panels;
 
   for (int it = 0;; ++it) {
     // work items in panel-major order: all tiles of panel 0, then panel 1, ...
-    const int work = s_work[it & 1];
+    const int4 wi = s_work[it & 1];
+    const int work = wi.x, row0 = wi.y, nrows = wi.z, k = wi.w;
     if (work >= total) break;
-    const int tile = work % a.n_tiles, panel = work / a.n_tiles;
-    const int row0 = __ldg(a.tile_row0 + tile);
-    const int nrows = __ldg(a.tile_row0 + tile + 1) - row0;
-    const int k = __ldg(a.tile_class + tile);
-    if (tid == 0) {
-      s_work[(it + 1) & 1] = atomicAdd(a.counter, 1);
-      s_ctr[0] = s_ctr[1] = s_ctr[2] = s_ctr[3] = s_ctr[4] = s_ctr[5] = 0;
-      if (MODE != MODE_INIT) {
-        // the tile panel of b_{k+1} -> buffer A, one bulk copy per sector (fibre pitch = n1) or
-        // per fibre (padded pitch)
+    const int panel = work / a.n_tiles;
+    if (tid == 0) s_ctr[0] = s_ctr[1] = s_ctr[2] = s_ctr[3] = 0;
+    if (MODE != MODE_INIT && warp == 0) {
+      // the tile panels of b_{k+1} -> buffer A and of the partial b_k -> buffer B: one bulk copy
+      // each, or one per fibre when the fibre pitch is padded
+      if (lane == 0) {
         fence_proxy_async();
-        mbar_expect_tx(&bar, (unsigned)nrows * 64u);
-        const double* src = a.X1 + panel * panel_stride + (size_t)row0 * kSecPanel;
+        mbar_expect_tx(&bar, 2u * (unsigned)nrows * 64u);
+      }
+      __syncwarp();
+      const size_t off = panel * panel_stride + (size_t)row0 * kSecPanel;
+      if (a.tab.rows_p[k] == nrows) {  // no padding: the whole tile is one run
+        if (lane < 2)
+          bulk_g2s(lane ? sB : sA, (lane ? a.Pk : a.X1) + off, (unsigned)nrows * 64u, &bar, pol_last);
+      } else {
         const int j_lo = k > G2 ? k - G2 : 0, j_hi = k < G1 ? k : G1;
         for (int j1 = j_lo; j1 <= j_hi; ++j1) {
           const int n1 = a.tab.n1[j1], n1p = a.tab.n1p[j1], n2 = a.tab.n2[k - j1];
           const int p0 = a.tab.sbase[k][j1], r0 = a.tab.srow[k][j1];
-          if (n1 == n1p) {
-            const unsigned bytes = (unsigned)(n1 * n2) * 64u;
-            for (unsigned at = 0; at < bytes; at += 32768u)
-              bulk_g2s(sA + (unsigned)r0 * 64u + at,
-                       reinterpret_cast<const char*>(src + (size_t)p0 * kSecPanel) + at,
-                       min(32768u, bytes - at), &bar, pol_last);
-          } else {
-            for (int i2 = 0; i2 < n2; ++i2)
-              bulk_g2s(sA + (unsigned)(r0 + i2 * n1p) * 64u, src + (size_t)(p0 + i2 * n1) * kSecPanel,
-                       (unsigned)n1 * 64u, &bar, pol_last);
+          for (int i = lane; i < 2 * n2; i += 32) {
+            const int i2 = i >> 1;
+            const double* src = ((i & 1) ? a.Pk : a.X1) + off + (size_t)(p0 + i2 * n1) * kSecPanel;
+            bulk_g2s(((i & 1) ? sB : sA) + (unsigned)(r0 + i2 * n1p) * 64u, src, (unsigned)n1 * 64u,
+                     &bar, pol_last);
           }
         }
       }
     }
     const uint4* meta = a.meta + (size_t)row0 * 2;
     const double* X1 = a.X1 + panel * panel_stride + 2 * q;
-    const double* Pk = a.Pk + panel * panel_stride + (size_t)row0 * kSecPanel + 2 * q;
     const double* V = a.V + panel * panel_stride + (size_t)row0 * kSecPanel + 2 * q;
     double* Bout = a.Bout + panel * panel_stride + 2 * q;
     double* Pout = a.Pout + panel * panel_stride + 2 * q;
     const uint16_t* units1 = a.units + (size_t)k * kSecMaxUnits;
     const uint16_t* units2 = a.units + (size_t)(M + 1 + k) * kSecMaxUnits;
-    __syncthreads();  // counters reset; the next work item is visible
+    // the rows of the row passes are dealt out statically: chunk c of 8 rows -> warp c mod warps
+    const int pos0 = warp * kTailRows + slot;
+    constexpr int kStride = kSecWarps * kTailRows;
+    __syncthreads();  // counters reset
     ++epoch;
+    // The next work item is claimed by the last warp (only its lane 0 waits for the atomic) and
+    // read after later barriers.
+    if (tid == kSecThreads - 32) s_work[(it + 1) & 1] = next_work();
 
-    // phase 2: B = O_l b_{k+1}, then b_k = P_k + pf (B + D b_{k+1} + cross terms)
+    // phase 2: B (= P_k) += pf O_l b_{k+1}, then b_k = B + pf (D b_{k+1} + cross terms)
     // phase 3: A = ps O_l b_k + qs b_k + rs b_{k+1}, then P_{k-1} = A + ps cross-group + cs V
-    // (one loop, so that the structured pass is instantiated once)
+    // (one loop, so that the structured passes are instantiated once)
 #pragma unroll 1
     for (int ph = 2; ph <= (MODE == MODE_LAST ? 2 : 3); ++ph) {
       if (MODE == MODE_INIT && ph == 2) {
         // ---- b_K = c_K V -> other layout and buffer B -----------------------------------------
-        for (int base = claim(&s_ctr[2], kTailRows, lane); base < nrows;
-             base = claim(&s_ctr[2], kTailRows, lane)) {
-          const int pos = base + slot;
-          if (pos < nrows) {
-            const uint4 m0 = ldg128(meta + (size_t)pos * 2);
-            double2 b = ldg128_stream(V + (size_t)pos * kSecPanel, pol_first);
-            b.x *= a.cK;
-            b.y *= a.cK;
-            stg128_stream(Bout + (size_t)m0.x * kSecPanel, b, pol_first);
-            sts128(sB + (m0.z >> 16) * 64u + 16u * q, b);
-          }
+        for (int pos = pos0; pos < nrows; pos += kStride) {
+          const uint4 m0 = ldg128(meta + (size_t)pos * 2);
+          double2 b = ldg128_stream(V + (size_t)pos * kSecPanel, pol_first);
+          b.x *= a.cK;
+          b.y *= a.cK;
+          stg128_stream(Bout + (size_t)m0.x * kSecPanel, b, pol_first);
+          sts128(sB + (m0.z >> 16) * 64u + 16u * q, b);
         }
         __syncthreads();
         ++epoch;
         continue;
       }
-      if (ph == 2) {
+      const bool p2 = ph == 2;
+      if (!p2) {  // row records and V of the next work item -> L2
+        const int4 wn = s_work[(it + 1) & 1];
+        if (wn.x < total) {
+          const int panel_n = wn.x / a.n_tiles, r0n = wn.y;
+          const unsigned bytes = (unsigned)wn.z * 64u;
+          const size_t off = panel_n * panel_stride + (size_t)r0n * kSecPanel;
+          const int per = (int)((bytes + 2047u) / 2048u);
+          l2_prefetch(a.meta + (size_t)r0n * 2, bytes / 2, tid, 0);
+          if (a.cs != 0.0) l2_prefetch(a.V + off, bytes, tid, (per + 1) / 2);
+        }
+      }
+      // Row passes are software-pipelined over three register sets (static indices: the loop
+      // body is unrolled three times): row records two iterations ahead, the global operands of
+      // a row (P_k or V, cross-cut partners) one iteration ahead; the first of them are
+      // requested before the structured passes, which hide their latency.
+      RowMeta m[kD];
+      m[0] = load_meta(meta, pos0, nrows, p2);
+      m[1] = load_meta(meta, pos0 + kStride, nrows, p2);
+      if (p2) {
         mbar_wait(&bar, parity);
         parity ^= 1u;
       }
-      const bool p2 = ph == 2;
-      structured_pass<G1, G2, NNN, JW>(a, k, units1, units2, &s_ctr[p2 ? 0 : 3], &s_ctr[p2 ? 1 : 4],
-                                       (p2 ? sA : sB) + 8u * l8, (p2 ? sB : sA) + 8u * l8,
-                                       p2 ? 1.0 : a.ps, p2 ? 0.0 : a.qs, p2 ? 0.0 : a.rs,
-                                       !p2 && MODE != MODE_INIT, epoch, lane);
-      int* const ctr = &s_ctr[p2 ? 2 : 5];
-      int base = claim(ctr, kTailRows, lane), base_n = claim(ctr, kTailRows, lane);
-      RowMeta nx = load_meta(meta, base + slot, nrows, p2);
+      structured_v1<G1, NNN, JW>(a, k, units1, &s_ctr[p2 ? 0 : 2], (p2 ? sA : sB) + 8u * l8,
+                                 (p2 ? sB : sA) + 8u * l8, p2 ? a.pf : a.ps, p2 ? 0.0 : a.qs,
+                                 p2 ? 1.0 : a.rs, p2 || MODE != MODE_INIT, epoch, lane);
       if (p2) {
-        for (; base < nrows; base = base_n, base_n = claim(ctr, kTailRows, lane)) {
-          const int pos = base + slot;
-          const bool active = pos < nrows;
-          const RowMeta m = nx;
-          nx = load_meta(meta, base_n + slot, nrows, true);
-          // the row's stream and its cross-cut partners (other tiles, from L2) fly during the rest
-          double2 pk = make_double2(0.0, 0.0);
-          if (active) pk = ldg128_stream(Pk + (size_t)pos * kSecPanel, pol_first);
-          const uint32_t c0 = m.m0.w, c1 = m.m1.x, c2 = m.m1.y;
-          const double2 h0 = ldg128_l2_if(X1 + (size_t)(c0 & kPosMask) * kSecPanel, c0 != kCrossNone);
-          const double2 h1 = ldg128_l2_if(X1 + (size_t)(c1 & kPosMask) * kSecPanel, c1 != kCrossNone);
-          const double2 h2 = ldg128_l2_if(X1 + (size_t)(c2 & kPosMask) * kSecPanel, c2 != kCrossNone);
-          const uint32_t own = (m.m0.z >> 16) * 64u + 16u * q;
-          double2 y = lds128(sB + own, epoch);
-          fma2(__hiloint2double((int)m.m1.w, (int)m.m1.z), lds128(sA + own, epoch), y);  // diagonal
-          cross_group(m, sA + 16u * q, a.t1, a.t2, epoch, y);
-          fma2(signed_coef(a.ccoef[(c0 >> kCrossPosBits) & 15u], c0), h0, y);
-          fma2(signed_coef(a.ccoef[(c1 >> kCrossPosBits) & 15u], c1), h1, y);
-          fma2(signed_coef(a.ccoef[(c2 >> kCrossPosBits) & 15u], c2), h2, y);
-          double2 b;
-          b.x = fma(a.pf, y.x, pk.x);
-          b.y = fma(a.pf, y.y, pk.y);
-          if (active) {
-            if (MODE == MODE_LAST) {
-              const int dst = __ldg(a.dst_nat + row0 + pos);
-              stg128_stream(a.W + (size_t)dst * a.w_ld + panel * kSecPanel + 2 * q, b, pol_first);
-            } else {
-              stg128_stream(Bout + (size_t)m.m0.x * kSecPanel, b, pol_first);
-              sts128(sB + own, b);
+        RowOperands o[kD];
+        o[0] = load_operands(m[0], X1);
+        structured_v2<G2, NNN, JW>(a, k, units2, &s_ctr[1], sA + 8u * l8, sB + 8u * l8, a.pf, epoch,
+                                   lane);
+#pragma unroll
+        for (int j = 2; j < kDM; ++j) m[j] = load_meta(meta, pos0 + j * kStride, nrows, true);
+#pragma unroll
+        for (int j = 1; j < kDO; ++j) o[j] = load_operands(m[j], X1);
+        for (int base = warp * kTailRows; base < nrows;) {  // warp-uniform loop control
+#pragma unroll
+          for (int j = 0; j < kD; ++j) {
+            const int pos = base + slot;
+            if (base >= nrows) break;
+            m[(j + kDM) % kD] = load_meta(meta, pos + kDM * kStride, nrows, true);
+            o[(j + kDO) % kD] = load_operands(m[(j + kDO) % kD], X1);
+            const uint32_t c0 = m[j].m0.w, c1 = m[j].m1.x, c2 = m[j].m1.y;
+            const uint32_t own = (m[j].m0.z >> 16) * 64u + 16u * q;
+            double2 y = make_double2(0.0, 0.0);
+            fma2(__hiloint2double((int)m[j].m1.w, (int)m[j].m1.z), lds128(sA + own, epoch), y);
+            cross_group(m[j], sA + 16u * q, a.t1, a.t2, epoch, y);
+            fma2(signed_coef(a.ccoef[(c0 >> kCrossPosBits) & 15u], c0), o[j].h0, y);
+            fma2(signed_coef(a.ccoef[(c1 >> kCrossPosBits) & 15u], c1), o[j].h1, y);
+            fma2(signed_coef(a.ccoef[(c2 >> kCrossPosBits) & 15u], c2), o[j].h2, y);
+            double2 b = lds128(sB + own, epoch);  // P_k + pf O_l b_{k+1}
+            b.x = fma(a.pf, y.x, b.x);
+            b.y = fma(a.pf, y.y, b.y);
+            if (pos < nrows) {
+              if (MODE == MODE_LAST) {
+                const int dst = __ldg(a.dst_nat + row0 + pos);
+                stg128_stream(a.W + (size_t)dst * a.w_ld + panel * kSecPanel + 2 * q, b, pol_first);
+              } else {
+                stg128_stream(Bout + (size_t)m[j].m0.x * kSecPanel, b, pol_first);
+                sts128(sB + own, b);
+              }
             }
+            base += kStride;
           }
         }
       } else {
-        for (; base < nrows; base = base_n, base_n = claim(ctr, kTailRows, lane)) {
-          const int pos = base + slot;
-          const bool active = pos < nrows;
-          const RowMeta m = nx;
-          nx = load_meta(meta, base_n + slot, nrows, false);
-          double2 v = make_double2(0.0, 0.0);
-          if (active && a.cs != 0.0) v = ldg128_stream(V + (size_t)pos * kSecPanel, pol_first);
-          const uint32_t own = (m.m0.z >> 16) * 64u + 16u * q;
-          double2 z = lds128(sA + own, epoch), g = make_double2(0.0, 0.0);
-          cross_group(m, sB + 16u * q, a.t1, a.t2, epoch, g);
-          z.x = fma(a.cs, v.x, fma(a.ps, g.x, z.x));
-          z.y = fma(a.cs, v.y, fma(a.ps, g.y, z.y));
-          if (active) stg128_stream(Pout + (size_t)m.m0.x * kSecPanel, z, pol_first);
+        const bool use_v = a.cs != 0.0;
+        double2 v[kD];
+        v[0] = load_stream_if(V, pos0, nrows, use_v, pol_first);
+        v[1] = load_stream_if(V, pos0 + kStride, nrows, use_v, pol_first);
+        structured_v2<G2, NNN, JW>(a, k, units2, &s_ctr[3], sB + 8u * l8, sA + 8u * l8, a.ps, epoch,
+                                   lane);
+#pragma unroll
+        for (int j = 2; j < kDM; ++j) {
+          m[j] = load_meta(meta, pos0 + j * kStride, nrows, false);
+          v[j] = load_stream_if(V, pos0 + j * kStride, nrows, use_v, pol_first);
+        }
+        for (int base = warp * kTailRows; base < nrows;) {  // warp-uniform loop control
+#pragma unroll
+          for (int j = 0; j < kD; ++j) {
+            const int pos = base + slot;
+            if (base >= nrows) break;
+            m[(j + kDM) % kD] = load_meta(meta, pos + kDM * kStride, nrows, false);
+            v[(j + kDM) % kD] = load_stream_if(V, pos + kDM * kStride, nrows, use_v, pol_first);
+            const uint32_t own = (m[j].m0.z >> 16) * 64u + 16u * q;
+            double2 z = lds128(sA + own, epoch), g = make_double2(0.0, 0.0);
+            cross_group(m[j], sB + 16u * q, a.t1, a.t2, epoch, g);
+            z.x = fma(a.cs, v[j].x, fma(a.ps, g.x, z.x));
+            z.y = fma(a.cs, v[j].y, fma(a.ps, g.y, z.y));
+            if (pos < nrows) stg128_stream(Pout + (size_t)m[j].m0.x * kSecPanel, z, pol_first);
+            base += kStride;
+          }
         }
       }
       __syncthreads();  // after phase 3: both buffers are free for the next tile

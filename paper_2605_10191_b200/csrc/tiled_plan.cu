@@ -405,8 +405,8 @@ void destroy_tiled_plan(TiledPlan* p) {
   delete p;
 }
 
-int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& terms, cudaStream_t st,
-                     TiledPlan** out) {
+int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& terms, bool sector,
+                     cudaStream_t st, TiledPlan** out) {
   *out = nullptr;
   const int L = basis->n_sites, n_up = basis->n_up;
   if (n_up < 0 || !basis->d_states)
@@ -475,10 +475,10 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
   rc = upload(&p->d_tile_rec0, rec0);
   if (rc) return rc;
 
-  // The sector sweep takes over when both layouts have uniform NN (+ NNN) bonds inside their
-  // tiles, at most three hops cross the cut and a kernel exists for this tile size.
+  // The sector sweep (POLFED_FORMAT_SECTOR) needs uniform NN (+ NNN) bonds inside the tiles of
+  // both layouts, at most three hops across the cut and a kernel for this tile size.
   SectorHost sh[2];
-  {
+  if (sector) {
     double t1[2], t2[2];
     bool nnn[2], jw[2];
     int cross_terms = 0;
@@ -488,14 +488,18 @@ int build_tiled_plan(const polfed_basis* basis, const std::vector<DevTerm>& term
                      sector_pattern(m, low[1], &t1[1], &t2[1], &nnn[1], &jw[1]) &&
                      nnn[0] == nnn[1] && (!nnn[0] || jw[0] == jw[1]) &&
                      sector_m_supported(m, nnn[0], jw[0]);
-    if (pat) {
+    if (!pat)
+      return fail(POLFED_EINVAL, "sector format: needs one amplitude on every (i,i+1) bond and none "
+                                 "or one on every (i,i+2) bond inside a tile, at most 3 hopping "
+                                 "terms across the cut, and ceil(n_sites/2) in the supported set");
+    {
       SectorPlan* sp = new (std::nothrow) SectorPlan;
       if (!sp) return fail(POLFED_ENOMEM, "tiled format: host allocation failed");
       p->sector = sp;
       sp->nnn = nnn[0];
       sp->jw = nnn[0] && jw[0];
       std::vector<uint16_t> units;
-      sector_geometry(m, /*pad=*/getenv("POLFED_SECTOR_PAD") != nullptr, sp, &units);
+      sector_geometry(m, /*pad=*/false, sp, &units);
       for (int l = 0; l < 2; ++l) {
         sp->lay[l].t1 = t1[l];
         sp->lay[l].t2 = t2[l];

@@ -1,6 +1,7 @@
-"""Parity of the tiled format (POLFED_FORMAT_TILED: alternating-layout Clenshaw pipeline with the
-tile in shared memory, include/polfed.h) against the CPU oracle's textbook Clenshaw on the same
-seeded inputs.  The tiled path must give the filter output of Eq. (51) PAPER.md:427-431 within
+"""Parity of the tiled formats (POLFED_FORMAT_TILED: alternating-layout Clenshaw pipeline with the
+tile in shared memory and per-row neighbour records; POLFED_FORMAT_SECTOR: the same pipeline with
+the tile-local hops applied from registers, include/polfed.h) against the CPU oracle's textbook
+Clenshaw on the same seeded inputs.  The tiled path must give the filter output of Eq. (51) PAPER.md:427-431 within
 rel l2 <= 1e-9 (north_star); it differs from the oracle only in summation order.
 """
 from __future__ import annotations
@@ -42,7 +43,12 @@ def tiled_filter(P, ham, a, b, coeffs, V):
 
 def build(P, n_sites, n_up, terms, fmt=None):
     basis = P.polfed_build_basis(n_sites, n_up)
+    if isinstance(fmt, str):
+        fmt = getattr(P, "FORMAT_" + fmt)
     return P.polfed_build_hamiltonian(basis, terms, fmt=P.FORMAT_TILED if fmt is None else fmt)
+
+
+FORMATS = ("TILED", "SECTOR")
 
 
 def gershgorin(H):
@@ -54,10 +60,11 @@ def gershgorin(H):
 FERMION = [(8, 4), (12, 6), (12, 3), (13, 6), (14, 9), (16, 8)]
 
 
+@pytest.mark.parametrize("fmt", FORMATS)
 @pytest.mark.parametrize("K", [1, 2, 3, 4, 9, 40])
 @pytest.mark.parametrize("s", (16, 32))
 @pytest.mark.parametrize("L,n_up", FERMION)
-def test_tiled_filter_random_coefficients(P, L, n_up, s, K):
+def test_tiled_filter_random_coefficients(P, L, n_up, s, K, fmt):
     rng = np.random.default_rng(100 * L + n_up)
     terms = workloads.fermion_terms(L, 1.0, 0.5, 1.0, rng.uniform(-2, 2, L))
     st = core.basis_states(L, n_up)
@@ -66,13 +73,14 @@ def test_tiled_filter_random_coefficients(P, L, n_up, s, K):
     a, b = 0.37, 1.05 * gershgorin(H)
     coeffs = np.random.default_rng(K).standard_normal(K + 1)
     want = core.clenshaw(H, a, b, coeffs, V)
-    got = tiled_filter(P, build(P, L, n_up, terms), a, b, coeffs, V)
+    got = tiled_filter(P, build(P, L, n_up, terms, fmt), a, b, coeffs, V)
     assert rel_l2(got, want) <= 1e-12
 
 
+@pytest.mark.parametrize("fmt", FORMATS)
 @pytest.mark.parametrize("config,L_override,K", [(5, 16, 200), (5, 18, 1000), (3, 14, 600),
                                                  (3, 16, None)])
-def test_tiled_filter_matches_oracle_on_workloads(P, config, L_override, K):
+def test_tiled_filter_matches_oracle_on_workloads(P, config, L_override, K, fmt):
     w = workloads.make_workload(config, L_override=L_override)
     _, H = core.hamiltonian(w)
     from oracle import lanczos
@@ -85,7 +93,7 @@ def test_tiled_filter_matches_oracle_on_workloads(P, config, L_override, K):
     coeffs = cheb.filter_coeffs(lam, K)
     V = workloads.start_block(H.n, w.s, seed=2000 + config, orthonormal=True)
     want = core.clenshaw(H, a, b, coeffs, V)
-    got = tiled_filter(P, build(P, w.n_sites, w.n_up, w.terms), a, b, coeffs, V)
+    got = tiled_filter(P, build(P, w.n_sites, w.n_up, w.terms, fmt), a, b, coeffs, V)
     assert K <= 5000 and rel_l2(got, want) <= 1e-9
 
 
@@ -118,6 +126,15 @@ def test_tiled_ineligible_requests_fail_loudly(P):
         basis = P.polfed_build_basis(n_sites, n_up)
         with pytest.raises(P.PolfedError):
             P.polfed_build_hamiltonian(basis, terms, fmt=P.FORMAT_TILED)
+    # the sector format wants uniform (i,i+1) / (i,i+2) bonds inside the tiles
+    for n_sites, n_up, terms in [(12, 6, [("HOPJW", i, i + 1, 1.0 + 0.1 * (i == 3)) for i in range(11)]),
+                                 (12, 6, [("HOPJW", i, i + 1, 1.0) for i in range(11) if i != 2]),
+                                 (12, 6, [("HOPJW", i, i + 1, 1.0) for i in range(11)]
+                                  + [("HOPJW", 0, 3, 0.5)]),
+                                 (22, 11, [("HOPJW", i, i + 1, 1.0) for i in range(21)])]:  # m = 11
+        basis = P.polfed_build_basis(n_sites, n_up)
+        with pytest.raises(P.PolfedError):
+            P.polfed_build_hamiltonian(basis, terms, fmt=P.FORMAT_SECTOR)
 
 
 def test_tiled_handle_still_serves_csr_entry_points(P):
@@ -138,7 +155,8 @@ def test_tiled_handle_still_serves_csr_entry_points(P):
 
 # ---- full BASELINE sizes, in the launch configuration bench.py times --------------------------
 
-def test_tiled_full_size_config3_matches_oracle(P):
+@pytest.mark.parametrize("fmt", FORMATS)
+def test_tiled_full_size_config3_matches_oracle(P, fmt):
     """Config 3 (XXZ L=20, D=184 756, s=16): the whole filter against the oracle, small K."""
     w = workloads.make_workload(3)
     _, H = core.hamiltonian(w)
@@ -146,7 +164,7 @@ def test_tiled_full_size_config3_matches_oracle(P):
     coeffs = np.random.default_rng(33).standard_normal(8)
     a, b = -0.4, 1.05 * gershgorin(H)
     want = core.clenshaw(H, a, b, coeffs, V)
-    got = tiled_filter(P, build(P, w.n_sites, w.n_up, w.terms), a, b, coeffs, V)
+    got = tiled_filter(P, build(P, w.n_sites, w.n_up, w.terms, fmt), a, b, coeffs, V)
     assert rel_l2(got, want) <= 1e-12
 
 
@@ -156,7 +174,8 @@ def _closure(states, rows, w):
     return np.unique(np.concatenate([rows, mini.col.astype(np.int64)])), mini
 
 
-def test_tiled_full_size_config5_sampled_rows(P):
+@pytest.mark.parametrize("fmt", FORMATS)
+def test_tiled_full_size_config5_sampled_rows(P, fmt):
     """Config 5 (D=10 400 600, s=32), K=3: first, two recurrence and last sweep of the tiled
     pipeline.  The oracle follows Eq. (51) on the rows that the sampled outputs depend on
     (two levels of matrix neighbours), one row at a time through its own CSR builder and SpMM;
@@ -164,7 +183,7 @@ def test_tiled_full_size_config5_sampled_rows(P):
     w = workloads.make_workload(5)
     states = core.basis_states(w.n_sites, w.n_up)
     n, s = int(states.shape[0]), w.s
-    ham = build(P, w.n_sites, w.n_up, w.terms)
+    ham = build(P, w.n_sites, w.n_up, w.terms, fmt)
     assert ham.n == n and ham.nnz == 275_407_888
     gen = torch.Generator(device="cuda").manual_seed(5105)
     V = torch.randn(n, s, dtype=torch.float64, device="cuda", generator=gen)
