@@ -228,8 +228,11 @@ int polfed_filter_coeffs(double a, double b, double sigma, int nev, double rho_r
 /* Extremal Ritz values of n_steps scalar Lanczos steps with full reorthogonalisation started
  * from d_v0 (n doubles, any nonzero vector; normalised internally) -- PAPER.md:86-125 (Eq. 1-6),
  * 276-278, 462.  Outputs (any may be NULL): *emin, *emax the extremal Ritz values,
- * *a = (emax+emin)/2, *b = (1+margin)(emax-emin)/2 (Eq. 31 widened by `margin`, R5; margin < 0
- * means the default 0.01).  n_steps <= 0 means 60 (R6); it is clipped to n.  Allocates
+ * *a = (hi+lo)/2, *b = (1+margin)(hi-lo)/2 (Eq. 31 widened by `margin`, R5; margin < 0
+ * means the default 0.01).  Ritz values lie inside the spectrum, so a and b are computed from
+ * the extremal Ritz values moved outwards by their residual norms beta_{m+1} |z_m| (Eq. 6, 16;
+ * zero once they have converged); *emin, *emax are the Ritz values themselves.
+ * n_steps <= 0 means 60 (R6); it is clipped to n.  Allocates
  * (n_steps+1) x n doubles of device scratch and frees it; synchronises `stream`. */
 int polfed_spectrum_bounds(const polfed_ham* ham, int n_steps, const double* d_v0, double margin,
                            void* stream, double* emin, double* emax, double* a, double* b);
@@ -259,32 +262,51 @@ typedef struct {
   double tol;             /* absolute bound on ||H x - lambda x||; <= 0: 1e-8 * max(|E_min|,|E_max|) */
   int32_t max_krylov_dim; /* <= 0: 5 nev + 8 s rounded up to a multiple of s (R10), capped by n and by free memory */
   int32_t check_every;    /* block steps between convergence checks; <= 0: adaptive (R9) */
-  int32_t K_override;     /* > 0: polynomial order; else Eq. (42)+(41) with the Gaussian DOS (R7) */
+  int32_t K_override;     /* > 0: polynomial order; else Eq. (42)+(41) with the density of states
+                             selected by `dos` (R7) */
   int32_t bounds_steps;   /* <= 0: 60 */
   double bounds_margin;   /* < 0: 0.01 */
   double a, b;            /* b > 0: rescaling parameters given, no Lanczos bounds run */
   int32_t sigma_is_rescaled; /* nonzero: sigma is the rescaled target lambda~ in (-1,1) (R8) */
-  int32_t reserved;
+  int32_t dos;            /* POLFED_DOS_GAUSSIAN (0): Eq. (34) from Tr H, Tr H^2;
+                             POLFED_DOS_KPM (1): Eq. (35)-(39) */
+  int32_t kpm_moments;    /* KPM: Chebyshev moments N; <= 0: 75 */
+  int32_t kpm_vectors;    /* KPM: columns R of d_kpm_block, a positive multiple of 4 (paper: 100) */
+  const double* d_kpm_block; /* KPM: n x kpm_vectors row-major DEVICE block of iid zero-mean
+                             unit-variance entries drawn by the caller (no RNG crosses the ABI) */
 } polfed_options;
+enum { POLFED_DOS_GAUSSIAN = 0, POLFED_DOS_KPM = 1 };
 
 typedef struct {
   double a, b, lambda_rescaled, e_min, e_max, tol;
-  int32_t K, block_steps, krylov_dim, n_converged, n_checks, reserved;
+  int32_t K, block_steps, krylov_dim, n_converged, n_checks;
+  int32_t K_gaussian;             /* order the Gaussian density of states gives (0 if not evaluated) */
   int64_t sparse_products;        /* fused launches, all phases */
   double seconds_bounds, seconds_filter, seconds_reorth, seconds_qr;
   double seconds_projected_eig;   /* dense eigen-decompositions of H_L and of the H-projection */
   double seconds_extraction, seconds_total;
+  double rho_gaussian, rho_kpm;   /* states per unit rescaled energy at the target (0: not evaluated) */
+  int32_t K_kpm;                  /* order the KPM density of states gives (0 if not evaluated) */
+  int32_t nev_window;             /* levels the filter window is sized for: nev + max(2, 10 %) */
+  double seconds_dos;             /* moments of the density-of-states estimate */
 } polfed_report;
 
 /* The nev eigenpairs of H nearest sigma (Sec. 4.6 steps 1-6):
  *   1. a, b from polfed_spectrum_bounds (first column of d_V0 as start) unless given;
- *   2. K from Eq. (40)-(42) with the Gaussian density of states Eq. (34) unless K_override;
+ *   2. K from Eq. (40)-(42) with the Gaussian density of states Eq. (34), or with the KPM
+ *      density Eq. (36) (options->dos = POLFED_DOS_KPM: the moments of polfed_kpm_moments over
+ *      the caller's random block, the Jackson-damped series of polfed_kpm_dos at the target),
+ *      unless K_override; the report carries both orders when both are evaluated;
  *   3. block Lanczos on P(H~) (Fig. 4): W = P(H~) V_k by polfed_filter_apply,
  *      A_k = V_k^T W, full reorthogonalisation against V_1..V_k (twice), W = V_{k+1} B_{k+1}
  *      by CholeskyQR2 (R17);
  *   4. at a check: eigen-decomposition of H_L (cuSOLVER syevd), the nev+s largest Ritz values,
  *      back-map u = V_{1:m} t (Eq. 43), Rayleigh-Ritz of H itself in span(u) (R21), residuals
- *      ||H x - E x||; stop when nev pairs have residual <= tol.
+ *      ||H x - E x||; stop when the nev extracted pairs nearest sigma all have residual <= tol
+ *      (a converged pair farther away never stands in for an unconverged nearer one) and lie in
+ *      the main lobe of the filter, P(lambda~_i) > Omega = 0.17613 (R4, R11).  The window is
+ *      sized for nev + max(2, 10 %) levels so that a density estimate a few per cent off still
+ *      leaves nev levels inside.
  * d_V0: n x s start block (need not be orthonormal; full column rank required).
  * Outputs: h_evals[nev] ascending, d_evecs n x nev row-major (column j pairs with h_evals[j]),
  * h_residuals[nev]; report may be NULL.  Returns POLFED_ENOCONV (outputs hold the best nev

@@ -47,10 +47,24 @@ def lanczos_extrema(H: core.CSR, v0: np.ndarray, m: int = 60):
     return float(ev[0]), float(ev[-1])
 
 
+def lanczos_extrema_residuals(H: core.CSR, v0: np.ndarray, m: int = 60):
+    """(E_min, E_max, r_min, r_max): the extremal Ritz values and their residual norms
+    ||H y - theta y|| = b_{m+1} |z_m| (Eq. 6; the scalar case of Eq. 16), z the eigenvector of
+    the Lanczos matrix and b_{m+1} the norm of the last residual vector."""
+    alpha, beta, _ = lanczos_tridiag(lambda X: core.spmm(H, X), v0, min(m, H.n))
+    k = alpha.shape[0]
+    T = np.diag(alpha) + np.diag(beta[:k - 1], 1) + np.diag(beta[:k - 1], -1)
+    ev, Z = np.linalg.eigh(T)
+    b_last = float(beta[k - 1])
+    return float(ev[0]), float(ev[-1]), b_last * abs(float(Z[k - 1, 0])), b_last * abs(float(Z[k - 1, -1]))
+
+
 def spectrum_bounds(H: core.CSR, v0: np.ndarray, m: int = 60, margin: float = 0.01):
-    """(E_min, E_max, a, b) with a, b from Eq. (31) widened by the margin (reading R5)."""
-    e_min, e_max = lanczos_extrema(H, v0, m)
-    a, b = cheb.rescale_params(e_min, e_max, margin)
+    """(E_min, E_max, a, b): the extremal Ritz values, and a, b of Eq. (31) computed from the
+    Ritz values moved outwards by their residual norms and widened by the margin (reading R5:
+    Ritz values lie inside the spectrum)."""
+    e_min, e_max, r_min, r_max = lanczos_extrema_residuals(H, v0, m)
+    a, b = cheb.rescale_params(e_min - r_min, e_max + r_max, margin)
     return e_min, e_max, a, b
 
 

@@ -50,19 +50,22 @@ class _Options(C.Structure):
     _fields_ = [("tol", C.c_double), ("max_krylov_dim", C.c_int32), ("check_every", C.c_int32),
                 ("K_override", C.c_int32), ("bounds_steps", C.c_int32),
                 ("bounds_margin", C.c_double), ("a", C.c_double), ("b", C.c_double),
-                ("sigma_is_rescaled", C.c_int32), ("reserved", C.c_int32)]
+                ("sigma_is_rescaled", C.c_int32), ("dos", C.c_int32), ("kpm_moments", C.c_int32),
+                ("kpm_vectors", C.c_int32), ("d_kpm_block", C.c_void_p)]
 
 
 class _Report(C.Structure):
     _fields_ = [("a", C.c_double), ("b", C.c_double), ("lambda_rescaled", C.c_double),
                 ("e_min", C.c_double), ("e_max", C.c_double), ("tol", C.c_double),
                 ("K", C.c_int32), ("block_steps", C.c_int32), ("krylov_dim", C.c_int32),
-                ("n_converged", C.c_int32), ("n_checks", C.c_int32), ("reserved", C.c_int32),
+                ("n_converged", C.c_int32), ("n_checks", C.c_int32), ("K_gaussian", C.c_int32),
                 ("sparse_products", C.c_int64),
                 ("seconds_bounds", C.c_double), ("seconds_filter", C.c_double),
                 ("seconds_reorth", C.c_double), ("seconds_qr", C.c_double),
                 ("seconds_projected_eig", C.c_double), ("seconds_extraction", C.c_double),
-                ("seconds_total", C.c_double)]
+                ("seconds_total", C.c_double), ("rho_gaussian", C.c_double),
+                ("rho_kpm", C.c_double), ("K_kpm", C.c_int32), ("nev_window", C.c_int32),
+                ("seconds_dos", C.c_double)]
 
 
 _lib = None
@@ -401,12 +404,20 @@ def polfed_block_lanczos_eigs(ham: Ham, sigma: float, nev: int, s: int, V0, *, t
                               max_krylov_dim: int = 0, check_every: int = 0, K_override: int = 0,
                               bounds_steps: int = 0, bounds_margin: float = -1.0, a: float = 0.0,
                               b: float = 0.0, sigma_is_rescaled: bool = False, stream=None,
-                              allow_unconverged: bool = False):
+                              allow_unconverged: bool = False, kpm_block=None,
+                              kpm_moments: int = 0):
     """The nev eigenpairs of H nearest sigma: (evals ndarray, evecs CUDA tensor n x nev,
-    residuals ndarray, report dict).  Raises PolfedError(ENOCONV) unless allow_unconverged."""
+    residuals ndarray, report dict).  Raises PolfedError(ENOCONV) unless allow_unconverged.
+    kpm_block (CUDA tensor n x R, R a multiple of 4): size K with the KPM density of states."""
     import torch
     opt = _Options(tol, max_krylov_dim, check_every, K_override, bounds_steps, bounds_margin, a, b,
-                   int(bool(sigma_is_rescaled)), 0)
+                   int(bool(sigma_is_rescaled)), 0, 0, 0, None)
+    if kpm_block is not None:
+        if (kpm_block.dim() != 2 or kpm_block.shape[0] != ham.n or kpm_block.dtype != torch.float64
+                or not kpm_block.is_cuda or not kpm_block.is_contiguous()):
+            raise ValueError("kpm_block must be a contiguous fp64 CUDA tensor n x R")
+        opt.dos, opt.kpm_moments, opt.kpm_vectors = 1, kpm_moments, int(kpm_block.shape[1])
+        opt.d_kpm_block = kpm_block.data_ptr()
     rep = _Report()
     evals = np.empty(nev, dtype=np.float64)
     resid = np.empty(nev, dtype=np.float64)

@@ -117,6 +117,18 @@ struct DenseEigh {
   }
 };
 
+// P(x) = sum_k c_k T_k(x) by the scalar Clenshaw recurrence (Eq. 50-51 with H~ -> x).
+double filter_value(const std::vector<double>& c, double x) {
+  double b1 = 0.0, b2 = 0.0;
+  for (size_t k = c.size() - 1; k >= 1; --k) {
+    const double t = c[k] + 2.0 * x * b1 - b2;
+    b2 = b1;
+    b1 = t;
+  }
+  return c[0] + x * b1 - b2;
+}
+constexpr double kOmega = 0.17613;  // sin(2.655)/2.655, the cutoff implied by Eq. (42) (R4)
+
 // ---- CholeskyQR on one n x s panel, in place ----------------------------------------------------
 struct PanelQR {
   int s;
@@ -183,6 +195,7 @@ int polfed_spectrum_bounds(const polfed_ham* ham, int n_steps, const double* d_v
   double* Phi = basis.f64();
   double* dC = coef.f64();
   std::vector<double> hC(m_max + 2), alpha, beta;
+  double b_last = 0.0;  // norm of the last residual vector
 
   // phi_1 = v0 / ||v0||
   POLFED_CUDA(cudaMemcpyAsync(Phi, d_v0, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, st));
@@ -217,6 +230,7 @@ int polfed_spectrum_bounds(const polfed_ham* ham, int n_steps, const double* d_v
     POLFED_CUDA(cudaMemcpyAsync(hC.data(), dC, sizeof(double), cudaMemcpyDeviceToHost, st));
     POLFED_CUDA(cudaStreamSynchronize(st));
     const double bnext = std::sqrt(std::max(hC[0], 0.0));
+    b_last = bnext;
     if (i + 1 == m_max || !(bnext > 1e-14 * std::max(1.0, std::fabs(alpha.back())))) break;
     beta.push_back(bnext);
     scale = 1.0 / bnext;
@@ -234,9 +248,12 @@ int polfed_spectrum_bounds(const polfed_ham* ham, int n_steps, const double* d_v
   DenseEigh eig;
   rc = eig.solve(m, T.data(), ev.data(), Z.data(), st);
   if (rc) return rc;
-  const double lo = ev.front(), hi = ev.back();
-  if (emin) *emin = lo;
-  if (emax) *emax = hi;
+  // Ritz values lie inside the spectrum: for a and b the extremal ones are moved outwards by
+  // their residual norms beta_{m+1} |last eigenvector component| (Eq. 6 / 16; reading R5)
+  if (emin) *emin = ev.front();
+  if (emax) *emax = ev.back();
+  const double lo = ev.front() - b_last * std::fabs(Z[(size_t)0 * m + (m - 1)]);
+  const double hi = ev.back() + b_last * std::fabs(Z[(size_t)(m - 1) * m + (m - 1)]);
   if (a) *a = 0.5 * (hi + lo);
   if (b) *b = 0.5 * (hi - lo) * (1.0 + margin);
   return POLFED_OK;
@@ -287,10 +304,16 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
   const double h_norm = std::max(std::fabs(e_min), std::fabs(e_max));
   const double tol = opt.tol > 0.0 ? opt.tol : 1e-8 * h_norm;
 
-  // -- step 2-3: order from the Gaussian density of states (Eq. 34, 40-42) and coefficients
+  // -- step 2-3: order from the density of states at the target (Eq. 34 or 35-39, then 40-42).
+  // The window is sized for 10 % more levels than asked for (at least 2 more): a density estimate
+  // that is a few per cent high would otherwise leave fewer than nev levels inside the main lobe
+  // and secondary-peak levels would fill the set (reading R4).
+  const int nev_window = nev + std::max(2, (nev + 9) / 10);
+  rep.nev_window = nev_window;
   int K = opt.K_override;
   double rho = 0.0;
   if (K <= 0) {
+    const double t0 = now_seconds();
     DeviceBuf mom;
     POLFED_CUDA(mom.alloc(2 * sizeof(double)));
     int rc = csr_moments(ham, mom.f64(), st);
@@ -300,19 +323,54 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
     POLFED_CUDA(cudaStreamSynchronize(st));
     const double mu = h_mom[0] / (double)n;
     const double var = h_mom[1] / (double)n - mu * mu;
-    if (!(var > 0.0)) return fail(POLFED_ERANGE, "polfed_block_lanczos_eigs: zero spectral width");
-    const double gam = std::sqrt(var);
-    const double rho_E = (double)n / (std::sqrt(2.0 * M_PI) * gam) *
+    if (var > 0.0) {
+      const double gam = std::sqrt(var);
+      rep.rho_gaussian = b_ * (double)n / (std::sqrt(2.0 * M_PI) * gam) *
                          std::exp(-(sigma_E - mu) * (sigma_E - mu) / (2.0 * var));
-    rho = rho_E * b_;  // states per unit rescaled energy
-    if (!(rho > 0.0)) return fail(POLFED_ERANGE, "polfed_block_lanczos_eigs: zero density of states at the target");
+      if (rep.rho_gaussian > 0.0)
+        polfed_filter_coeffs(a_, b_, sigma_E, nev_window, rep.rho_gaussian, 0, &rep.K_gaussian, nullptr, 0);
+    }
+    if (opt.dos == POLFED_DOS_KPM) {
+      // Eq. (37)-(38): moments averaged over the caller's random vectors, in chunks of at most 32
+      const int n_mom = opt.kpm_moments > 0 ? opt.kpm_moments : 75;
+      const int n_vec = opt.kpm_vectors;
+      if (!opt.d_kpm_block || n_vec < 4 || n_vec % 4 != 0)
+        return fail(POLFED_EINVAL, "polfed_block_lanczos_eigs: POLFED_DOS_KPM needs d_kpm_block with a "
+                                   "positive multiple of 4 columns");
+      DeviceBuf chunk, kwork;
+      POLFED_CUDA(chunk.alloc(sizeof(double) * (size_t)n * 32));
+      POLFED_CUDA(kwork.alloc(polfed_kpm_workspace_bytes(n, 32, n_mom)));
+      std::vector<double> mu_avg(n_mom, 0.0), mu_c(n_mom);
+      for (int c0 = 0; c0 < n_vec;) {
+        const int left = n_vec - c0;
+        const int sc = left >= 32 ? 32 : (left >= 16 ? 16 : (left >= 8 ? 8 : 4));
+        POLFED_CUDA(cudaMemcpy2DAsync(chunk.p, sizeof(double) * sc, opt.d_kpm_block + c0,
+                                      sizeof(double) * n_vec, sizeof(double) * sc, (size_t)n,
+                                      cudaMemcpyDeviceToDevice, st));
+        rc = polfed_kpm_moments(ham, a_, b_, n_mom, sc, chunk.f64(), kwork.p, mu_c.data(), stream);
+        if (rc) return rc;
+        for (int i = 0; i < n_mom; ++i) mu_avg[i] += mu_c[i] * sc / n_vec;
+        rep.sparse_products += n_mom;
+        c0 += sc;
+      }
+      rc = polfed_kpm_dos(mu_avg.data(), n_mom, &lam, 1, &rep.rho_kpm);
+      if (rc) return rc;
+      if (rep.rho_kpm > 0.0)
+        polfed_filter_coeffs(a_, b_, sigma_E, nev_window, rep.rho_kpm, 0, &rep.K_kpm, nullptr, 0);
+      rho = rep.rho_kpm;
+    } else {
+      rho = rep.rho_gaussian;
+    }
+    rep.seconds_dos = now_seconds() - t0;
+    if (!(rho > 0.0))
+      return fail(POLFED_ERANGE, "polfed_block_lanczos_eigs: zero density of states at the target");
   }
   int K_out = 0;
-  int rc = polfed_filter_coeffs(a_, b_, sigma_E, nev, rho, K, &K_out, nullptr, 0);
+  int rc = polfed_filter_coeffs(a_, b_, sigma_E, nev_window, rho, K, &K_out, nullptr, 0);
   if (rc) return rc;
   K = K_out;
   std::vector<double> coeffs((size_t)K + 1);
-  rc = polfed_filter_coeffs(a_, b_, sigma_E, nev, 0.0, K, &K_out, coeffs.data(), K + 1);
+  rc = polfed_filter_coeffs(a_, b_, sigma_E, nev_window, 0.0, K, &K_out, coeffs.data(), K + 1);
   if (rc) return rc;
 
   // -- sizes and device memory
@@ -391,6 +449,11 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
     }
     POLFED_CUDA(cudaStreamSynchronize(st));
     rep.seconds_reorth += now_seconds() - t0;
+    if (k == 1)  // a spectrum that sticks out of [-1, 1] makes the recurrence grow like cosh(K acosh|x|)
+      for (int i = 0; i < s * s; ++i)
+        if (!std::isfinite(hC[i]))
+          return fail(POLFED_ERANGE, "polfed_block_lanczos_eigs: the filtered block is not finite "
+                                     "(spectrum outside [a - b, a + b]?)");
     const size_t o = (size_t)(k - 1) * s;
     for (int i = 0; i < s; ++i)
       for (int j = 0; j < s; ++j)
@@ -504,9 +567,17 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
     std::vector<int> good;
     for (int c : order)
       if (res[c] <= tol) good.push_back(c);
-    rep.n_converged = (int)std::min<size_t>(good.size(), (size_t)nev);
+    // done only when the nev extracted pairs nearest sigma are all converged (a converged pair
+    // farther away must not stand in for an unconverged nearer one) and lie inside the main lobe
+    // of the filter, P(lambda~_i) > Omega: levels on a secondary peak
+    // (P <= 0.128) are true eigenpairs too, but the set would not be contiguous
+    int n_lead = 0;
+    while (n_lead < wp && res[order[n_lead]] <= tol &&
+           filter_value(coeffs, (Eg[order[n_lead]] - a_) / b_) > kOmega)
+      ++n_lead;
+    rep.n_converged = std::min(n_lead, nev);
     std::vector<int> sel;
-    const bool done = (int)good.size() >= nev;
+    const bool done = n_lead >= nev;
     if (done) {
       sel.assign(good.begin(), good.begin() + nev);
     } else {
@@ -535,7 +606,7 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
       status = POLFED_OK;
       break;
     }
-    const int missing = nev - (int)good.size();
+    const int missing = nev - std::min(n_lead, nev);
     next_check = opt.check_every > 0 ? k + opt.check_every : k + std::max(1, (missing + 2 * s - 1) / (2 * s));
   }
 

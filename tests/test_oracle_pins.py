@@ -444,6 +444,30 @@ def test_lanczos_extrema_converge_to_spectrum_edges():
     assert (ev[0] - a) / b > -1.0 and (ev[-1] - a) / b < 1.0
 
 
+def test_lanczos_residual_norm_identity_and_widened_bounds():
+    """Eq. (6) / (16) for the scalar recurrence: ||H y - theta y|| = b_{m+1} |z_m| for a Ritz pair
+    (y = Phi z); spectrum_bounds (reading R5) moves the extremal Ritz values outwards by it, so an
+    unconverged run (m = 8) still has a true eigenvalue inside each widened end."""
+    st, H = core.hamiltonian(workloads.make_workload(1))
+    v0 = workloads.start_block(H.n, 1, 6)[:, 0]
+    m = 8
+    alpha, beta, Phi = lanczos.lanczos_tridiag(lambda X: core.spmm(H, X), v0, m)
+    T = np.diag(alpha) + np.diag(beta[:m - 1], 1) + np.diag(beta[:m - 1], -1)
+    th, Z = np.linalg.eigh(T)
+    e_min, e_max, r_min, r_max = lanczos.lanczos_extrema_residuals(H, v0, m)
+    for j, r in ((0, r_min), (m - 1, r_max)):
+        y = Phi @ Z[:, j]
+        direct = np.linalg.norm(core.spmm(H, y.reshape(-1, 1)).reshape(-1) - th[j] * y)
+        assert abs(direct - r) <= 1e-10 * max(1.0, abs(th[j]))
+    assert r_min > 1e-3 and r_max > 1e-3                      # not converged after 8 steps
+    ev = np.linalg.eigvalsh(H.to_dense())
+    assert np.min(np.abs(ev - e_min)) <= r_min + 1e-12        # an eigenvalue within the residual
+    assert np.min(np.abs(ev - e_max)) <= r_max + 1e-12
+    g_min, g_max, a, b = lanczos.spectrum_bounds(H, v0, m, 0.0)
+    assert (g_min, g_max) == (e_min, e_max)
+    assert abs((a - b) - (e_min - r_min)) <= 1e-12 and abs((a + b) - (e_max + r_max)) <= 1e-12
+
+
 def test_block_lanczos_invariants():
     A, H = random_symmetric_csr(96, 0.2, 21)
     s, m = 4, 8
