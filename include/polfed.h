@@ -129,9 +129,21 @@ int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_ter
  * 4 <= n_sites <= 26, no dense block,
  * off-diagonal terms of kind EXCH or HOPJW only, at most 4 distinct |amp| and 24 hops per state
  * inside a tile.  Used by polfed_filter_apply for s in {16, 32}; every other entry point uses
- * the CSR.  The tiled sweeps keep a tile counter inside the handle: do not run two filter
- * applications on the same POLFED_FORMAT_TILED handle concurrently (two streams or two threads);
- * back-to-back calls on one stream are fine. */
+ * the CSR.  On this path d_V and d_W must be 32-byte and d_work 128-byte aligned (POLFED_EINVAL
+ * otherwise).  All mutable state of a filter application (tile counters included) lives in the
+ * caller's d_work, so one handle may serve several streams at once with distinct workspaces.
+ *
+ * POLFED_FORMAT_SECTOR: the same two-layout pipeline for chains whose tile-local hops are one
+ * amplitude on every bond (i, i+1) and none or one amplitude on every bond (i, i+2) (EXCH, or
+ * HOPJW with its Jordan-Wigner sign), e.g. config 5 (t, t') and the XXZ chains (J/2).  The m tile
+ * sites are split into two groups; a lane group holds all rows that differ only inside one group
+ * (at most C(7,3) = 35) in registers and applies that group's hops as a compile-time operator, so
+ * shared memory is touched about 5 times per row and phase instead of once per stored entry; only
+ * the bonds between the groups and across the tile cut remain per-row gathers.  Blocks are
+ * streamed as 8-column panels (64-byte rows), the tile twice in shared memory.  Requirements
+ * beyond POLFED_FORMAT_TILED's (else POLFED_EINVAL): the bond pattern above in both row orders,
+ * at most 3 hopping terms across the cut, ceil(n_sites/2) in {4..9, 13} (chains with (i, i+2)
+ * bonds) or {6, 7, 8, 10} (without).  Same alignment rules and workspace ownership. */
 
 /* POLFED_FORMAT_SELL (SELL-C-sigma, C = 8, sigma = 128): besides the CSR, the handle keeps the
  * rows sorted by falling length inside windows of 128 rows, cut into slices of 8 rows stored
@@ -182,8 +194,8 @@ int polfed_fused_step(const polfed_ham* ham, int s, double p, double q, double r
 /* 2 * n * s * sizeof(double): the two auxiliary blocks of PAPER.md:431. */
 size_t polfed_filter_workspace_bytes(int64_t n, int s);
 /* Workspace polfed_filter_apply needs for this handle: the value above for a CSR handle; for a
- * POLFED_FORMAT_TILED handle and s in {16, 32}: 6 blocks (two b/partial pairs, V in both row
- * orders) plus a per-CTA tile scratch. */
+ * POLFED_FORMAT_TILED or _SECTOR handle and s in {16, 32}: 6 blocks (two b/partial pairs, V in
+ * both row orders) plus (tiled) a per-CTA tile scratch and the tile counters. */
 size_t polfed_filter_workspace_bytes_ham(const polfed_ham* ham, int s);
 
 /* W = sum_{k=0..K} h_coeffs[k] T_k(H~) V,  H~ = (H - a)/b, by the Clenshaw recurrence
@@ -200,8 +212,10 @@ size_t polfed_filter_workspace_bytes_ham(const polfed_ham* ham, int s);
 int polfed_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,
                         int s, const double* d_V, double* d_W, void* d_work, void* stream);
 
-/* Same operation on HOST blocks: allocates device blocks, copies h_V up, runs
- * polfed_filter_apply, copies W down into h_W, frees, synchronises.  The end-to-end entry. */
+/* Same operation on HOST blocks: takes device blocks from the device's stream-ordered memory
+ * pool (cudaMallocAsync; the pool's release threshold is raised so that later calls reuse them
+ * instead of allocating), copies h_V up, runs polfed_filter_apply, copies W down into h_W,
+ * returns the blocks to the pool, synchronises.  The end-to-end entry. */
 int polfed_filter_apply_host(const polfed_ham* ham, double a, double b, int K,
                              const double* h_coeffs, int s, const double* h_V, double* h_W,
                              void* stream);

@@ -123,6 +123,7 @@ def _stream(stream=None) -> Optional[int]:
     if stream is None:
         import torch
         stream = torch.cuda.current_stream().cuda_stream
+    stream = getattr(stream, "cuda_stream", stream)   # a torch.cuda.Stream or a raw handle
     return C.c_void_p(int(stream)) if stream else None
 
 

@@ -11,11 +11,16 @@ namespace polfed {
 // saturated; they are never reached because dim < 2^31 is enforced.
 static __constant__ uint64_t c_binom[kBinomDim * kBinomDim];
 static uint64_t h_binom[kBinomDim * kBinomDim];
-static bool g_binom_ready = false;
+static bool g_binom_host_ready = false;
+static unsigned long long g_binom_device_mask = 0;  // devices (ordinal < 64) that hold the table
 
+// The host table is filled once; the constant-memory copy is per device, so it is uploaded on
+// the first use on every device.
 static int ensure_binomials() {
-  if (g_binom_ready) return POLFED_OK;
-  for (int n = 0; n < kBinomDim; ++n)
+  int dev = 0;
+  POLFED_CUDA(cudaGetDevice(&dev));
+  if (g_binom_host_ready && dev < 64 && ((g_binom_device_mask >> dev) & 1ull)) return POLFED_OK;
+  for (int n = 0; n < kBinomDim && !g_binom_host_ready; ++n)
     for (int k = 0; k < kBinomDim; ++k) {
       uint64_t v;
       if (k == 0) v = 1;
@@ -26,8 +31,9 @@ static int ensure_binomials() {
       }
       h_binom[n * kBinomDim + k] = v;
     }
+  g_binom_host_ready = true;
   POLFED_CUDA(cudaMemcpyToSymbol(c_binom, h_binom, sizeof h_binom));
-  g_binom_ready = true;
+  if (dev < 64) g_binom_device_mask |= 1ull << dev;
   return POLFED_OK;
 }
 

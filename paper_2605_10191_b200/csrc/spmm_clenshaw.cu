@@ -308,6 +308,12 @@ int polfed_filter_apply(const polfed_ham* ham, double a, double b, int K, const 
     return fail(POLFED_EINVAL, "polfed_filter_apply: NULL block");
   if (!polfed::aligned16(d_V) || !polfed::aligned16(d_W) || !polfed::aligned16(d_work))
     return fail(POLFED_EINVAL, "polfed_filter_apply: blocks must be 16-byte aligned");
+  // the tiled sweeps move 32-byte pieces of V and W and bulk-copy 128-byte rows of the workspace
+  if (K >= 1 && polfed::tiled_supports(ham, s) &&
+      (((reinterpret_cast<uintptr_t>(d_V) | reinterpret_cast<uintptr_t>(d_W)) & 31u) != 0 ||
+       (reinterpret_cast<uintptr_t>(d_work) & 127u) != 0))
+    return fail(POLFED_EINVAL, "polfed_filter_apply: on a tiled or sector handle d_V and d_W must be "
+                               "32-byte and d_work 128-byte aligned");
   const size_t len = (size_t)ham->n * s;
   const size_t bytes = len * sizeof(double);
   const size_t work_bytes = polfed_filter_workspace_bytes_ham(ham, s);
@@ -351,20 +357,31 @@ int polfed_filter_apply_host(const polfed_ham* ham, double a, double b, int K,
   if (!h_V || !h_W) return fail(POLFED_EINVAL, "polfed_filter_apply_host: NULL block");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const size_t bytes = (size_t)ham->n * s * sizeof(double);
-  double* d_all = nullptr;  // V | W | work
-  POLFED_CUDA(cudaMalloc(&d_all, 2 * bytes + polfed_filter_workspace_bytes_ham(ham, s)));
-  const size_t len = bytes / sizeof(double);
-  double* d_V = d_all;
-  double* d_W = d_all + len;
-  double* d_work = d_all + 2 * len;
+  const size_t pitch = (bytes + 127) / 128 * 128;  // every sub-buffer starts on a 128-byte boundary
+  // V | W | work from the stream-ordered pool: after the first call the blocks are reused, not
+  // allocated (the pool keeps them: release threshold raised once per device)
+  {
+    int dev = 0;
+    POLFED_CUDA(cudaGetDevice(&dev));
+    cudaMemPool_t pool;
+    POLFED_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
+    unsigned long long keep = ~0ull;
+    POLFED_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+  }
+  char* d_all = nullptr;
+  POLFED_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&d_all),
+                              2 * pitch + polfed_filter_workspace_bytes_ham(ham, s), st));
+  double* d_V = reinterpret_cast<double*>(d_all);
+  double* d_W = reinterpret_cast<double*>(d_all + pitch);
+  void* d_work = d_all + 2 * pitch;
   int rc = POLFED_OK;
   cudaError_t e = cudaMemcpyAsync(d_V, h_V, bytes, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) {
     rc = polfed_filter_apply(ham, a, b, K, h_coeffs, s, d_V, d_W, d_work, stream);
     if (rc == POLFED_OK) e = cudaMemcpyAsync(h_W, d_W, bytes, cudaMemcpyDeviceToHost, st);
   }
+  cudaFreeAsync(d_all, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cudaFree(d_all);
   if (rc) return rc;
   if (e != cudaSuccess)
     return fail(POLFED_ECUDA, "polfed_filter_apply_host: %s", cudaGetErrorString(e));

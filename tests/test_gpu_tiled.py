@@ -137,6 +137,64 @@ def test_tiled_ineligible_requests_fail_loudly(P):
             P.polfed_build_hamiltonian(basis, terms, fmt=P.FORMAT_SECTOR)
 
 
+@pytest.mark.parametrize("fmt", FORMATS)
+def test_tiled_misaligned_blocks_are_rejected_not_faulted(P, fmt):
+    """16-byte aligned views that are not 32/128-byte aligned must give POLFED_EINVAL on
+    the tiled paths (they use 256-bit accesses and 128-byte bulk copies), not a device fault."""
+    w = workloads.make_workload(5, L_override=12)
+    ham = build(P, w.n_sites, w.n_up, w.terms, fmt)
+    n, s = ham.n, 16
+    need = P.polfed_filter_workspace_bytes_ham(ham, s) // 8
+    pool = torch.zeros(2 * n * s + need + 64, dtype=torch.float64, device="cuda")
+    coeffs = np.array([0.3, 0.2, 0.1])
+    def blocks(off_v, off_w, off_work):
+        V = pool[off_v: off_v + n * s].view(n, s)
+        W = pool[n * s + 16 + off_w: n * s + 16 + off_w + n * s].view(n, s)
+        work = pool[2 * n * s + 32 + off_work: 2 * n * s + 32 + off_work + need]
+        return V, W, work
+    for offs in ((2, 0, 0), (0, 2, 0), (0, 0, 2), (0, 0, 8)):      # 16-byte steps = 2 doubles
+        V, W, work = blocks(*offs)
+        with pytest.raises(P.PolfedError) as err:
+            P.polfed_filter_apply(ham, 0.0, 20.0, coeffs, s, V, W, work)
+        assert err.value.code == P.binding.EINVAL
+    V, W, work = blocks(0, 0, 0)
+    pool.normal_()
+    P.polfed_filter_apply(ham, 0.0, 20.0, coeffs, s, V, W, work)      # aligned: fine
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(W).all())
+
+
+def test_tiled_two_streams_share_one_handle(P):
+    """The tile counters live in the workspace: two filter applications on one handle, enqueued on
+    two streams with their own workspaces, give the same result as one after the other."""
+    w = workloads.make_workload(5, L_override=16)
+    ham = build(P, w.n_sites, w.n_up, w.terms)
+    n, s = ham.n, 32
+    need = P.polfed_filter_workspace_bytes_ham(ham, s) // 8
+    gen = torch.Generator(device="cuda").manual_seed(9)
+    Vs = [torch.randn(n, s, dtype=torch.float64, device="cuda", generator=gen) for _ in range(2)]
+    coeffs = np.random.default_rng(3).standard_normal(30)
+    ref = []
+    for V in Vs:
+        W = torch.empty_like(V)
+        work = torch.empty(need, dtype=torch.float64, device="cuda")
+        P.polfed_filter_apply(ham, 0.1, 20.0, coeffs, s, V, W, work)
+        ref.append(W)
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs, works = [], []
+    for V, st in zip(Vs, streams):
+        with torch.cuda.stream(st):
+            W = torch.empty_like(V)
+            work = torch.empty(need, dtype=torch.float64, device="cuda")
+            P.polfed_filter_apply(ham, 0.1, 20.0, coeffs, s, V, W, work, stream=st)
+            outs.append(W)
+            works.append(work)
+    torch.cuda.synchronize()
+    for W, R in zip(outs, ref):
+        assert torch.equal(W, R)
+
+
 def test_tiled_handle_still_serves_csr_entry_points(P):
     w = workloads.make_workload(5, L_override=12)
     _, H = core.hamiltonian(w)
