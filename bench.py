@@ -174,21 +174,38 @@ def oracle_time_steps(mini, w, B1, B2, V, T, n_steps: int):
     return time.perf_counter() - t0
 
 
-def cpu_baseline(config: int, budget_s: float = 15.0):
-    """Oracle recurrence steps (orc_clenshaw_step, as it stands) on the first rows of the workload."""
+def cpu_baseline(config: int, budget_s: float = 12.0):
+    """Oracle recurrence steps (orc_clenshaw_step, as it stands) on the first rows of the workload,
+    on all host cores and (the same library, OpenMP told to use one thread) on a single core."""
+    import ctypes
     from oracle import core
     rows = {1: 924, 2: 12870, 3: 184756, 4: 262144, 5: 262144}[config]
     w, n, mini, B1, B2, V, T = oracle_sample(config, rows, seed=7000 + config)
-    oracle_time_steps(mini, w, B1, B2, V, T, 1)
-    t1 = oracle_time_steps(mini, w, B1, B2, V, T, 2) / 2
-    n_steps = int(max(3, min(200, budget_s / max(t1, 1e-6))))
-    t = oracle_time_steps(mini, w, B1, B2, V, T, n_steps) / n_steps
     by = step_bytes(mini.n, mini.nnz, w.s)
-    return {"value": by / t / 1e9, "unit": UNIT, "cores": core.num_threads(), "kind": "oracle",
+
+    def timed(budget):
+        oracle_time_steps(mini, w, B1, B2, V, T, 1)
+        t1 = oracle_time_steps(mini, w, B1, B2, V, T, 2) / 2
+        n_steps = int(max(3, min(200, budget / max(t1, 1e-6))))
+        return oracle_time_steps(mini, w, B1, B2, V, T, n_steps) / n_steps, n_steps
+
+    cores = core.num_threads()
+    t, n_steps = timed(budget_s)
+    single = None
+    try:
+        gomp = ctypes.CDLL("libgomp.so.1")
+        gomp.omp_set_num_threads(1)
+        t_single, n_single = timed(budget_s / 2)
+        gomp.omp_set_num_threads(cores)
+        single = {"value": by / t_single / 1e9, "unit": UNIT, "cores": 1, "steps": n_single,
+                  "ms_per_recurrence_step": t_single * 1e3}
+    except OSError:
+        pass
+    return {"value": by / t / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{n_steps} recurrence steps (orc_clenshaw_step) on rows [0,{mini.n}) of "
                       f"{WORKLOAD_NAMES[config]} (nnz {mini.nnz}), full-size X block, "
                       f"{t * 1e3:.2f} ms/step",
-            "ms_per_recurrence_step": t * 1e3}
+            "ms_per_recurrence_step": t * 1e3, "single_thread": single}
 
 
 def run_reference(args):
@@ -251,10 +268,13 @@ def run_cuda(args):
     # auto: the flip format (matrix-free rows) for full-space models it supports (config 4)
     flip = args.format == "flip" or (args.format == "auto" and w.n_up < 0 and w.s in (8, 16, 32)
                                      and all(t[0] in ("XX", "Z", "ZZ") for t in w.terms))
-    fmt_name = "tiled" if tiled else ("flip" if flip else ("sell" if args.format == "sell" else "csr"))
+    fmt_name = "tiled" if tiled else ("flip" if flip else
+                                      (args.format if args.format in ("sell", "sector") else "csr"))
     ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense,
                                      fmt={"tiled": P.FORMAT_TILED, "flip": P.FORMAT_FLIP,
-                                          "sell": P.FORMAT_SELL, "csr": P.FORMAT_CSR}[fmt_name])
+                                          "sell": P.FORMAT_SELL, "csr": P.FORMAT_CSR,
+                                          "sector": P.FORMAT_SECTOR}[fmt_name])
+    tiled = tiled or fmt_name == "sector"     # same launch structure and timing method
     torch.cuda.synchronize()
     build_s = time.perf_counter() - t0
     n, nnz, s, K = ham.n, ham.nnz, w.s, args.order
@@ -366,7 +386,7 @@ def run_cuda(args):
             "clocks": clocks.summary(),
             "roofline": {"bound": "hbm",
                          "kernel": {"tiled": "tiled_sweep_kernel", "flip": "flip_step_kernel",
-                                    "sell": "sell_step_kernel",
+                                    "sell": "sell_step_kernel", "sector": "sector_sweep_kernel",
                                     "csr": "fused_step_kernel"}[fmt_name], "achieved": achieved,
                          "peak": peak, "peak_source": peak_src, "unit": UNIT,
                          "frac": achieved / peak, "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS,
@@ -374,8 +394,15 @@ def run_cuda(args):
                          "traffic": recorded_traffic(WORKLOAD_NAMES[args.config]
                                                     + "/" + fmt_name)},
         }
-        if world == 1 and args.eigs:
+        if world == 1 and args.per_config:
             del Vh, Wh, V
+            torch.cuda.empty_cache()
+            todo = [(int(c), "") for c in args.per_config.split(",") if c and int(c) != args.config]
+            line["per_config"] = [hot_path_on_config(P, c, peak, f) for c, f in todo]
+            if args.config == 5 and fmt_name == "tiled":   # the evaluated alternative (DESIGN 5d)
+                line["per_config"].append(hot_path_on_config(P, 5, peak, "sector"))
+            torch.cuda.empty_cache()
+        if world == 1 and args.eigs:
             torch.cuda.empty_cache()
             line["seconds_to_nev"] = [time_to_nev(P, int(c)) for c in args.eigs.split(",") if c]
         if world == 1 and not args.no_cpu_baseline:
@@ -385,6 +412,72 @@ def run_cuda(args):
         dist.barrier()
         dist.destroy_process_group()
     return 0
+
+
+def hot_path_on_config(P, config: int, peak: float, fmt_name: str = ""):
+    """The fused launch alone on another BASELINE config: format, ms per
+    launch (CUDA events over back-to-back launches on the launching stream), algorithmic GB/s and
+    the fraction of the measured and of the nominal HBM rate, and filter steps/s of one filter
+    application.  Configs 1-3 fit L2 (noted: the filter re-reads its working set by design)."""
+    import torch
+    w = workloads.make_workload(config)
+    basis = P.polfed_build_basis(w.n_sites, w.n_up)
+    flip = w.n_up < 0 and w.s in (8, 16, 32) and all(t[0] in ("XX", "Z", "ZZ") for t in w.terms)
+    fmt_name = fmt_name or ("flip" if flip else "csr")
+    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense,
+                                     fmt=getattr(P, "FORMAT_" + fmt_name.upper()))
+    n, nnz, s = ham.n, ham.nnz, w.s
+    a, b = 0.0, 80.0
+    gen = torch.Generator(device="cuda").manual_seed(2000 + config)
+    V = torch.randn(n, s, dtype=torch.float64, device="cuda", generator=gen)
+    W = torch.empty_like(V)
+    work = torch.empty(P.polfed_filter_workspace_bytes_ham(ham, s) // 8, dtype=torch.float64,
+                       device="cuda")
+    by = step_bytes(n, nnz, s)
+    n_l = max(20, min(2000, int(0.25e12 / max(by, 1))))
+    k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if fmt_name in ("tiled", "sector"):
+        t_pair = []
+        for cc in (np.full(9, 1e-3), np.full(9 + n_l, 1e-3)):
+            P.polfed_filter_apply(ham, a, b, cc, s, V, W, work)
+            k0.record()
+            P.polfed_filter_apply(ham, a, b, cc, s, V, W, work)
+            k1.record()
+            torch.cuda.synchronize()
+            t_pair.append(k0.elapsed_time(k1))
+        launch_ms = (t_pair[1] - t_pair[0]) / n_l
+    else:
+        B1, B2 = work[: n * s].view(n, s), work[n * s: 2 * n * s].view(n, s)
+        B1.copy_(V)
+        B2.copy_(V)
+        for _ in range(5):
+            P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, -1.0, 1e-3, B1, B2, V, B2)
+            B1, B2 = B2, B1
+        k0.record()
+        for _ in range(n_l):
+            P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, -1.0, 1e-3, B1, B2, V, B2)
+            B1, B2 = B2, B1
+        k1.record()
+        torch.cuda.synchronize()
+        launch_ms = k0.elapsed_time(k1) / n_l
+    # one whole filter application (the library call): filter steps per second
+    K = w.K_fixed or 1000
+    coeffs = np.full(K + 1, 1e-3)
+    P.polfed_filter_apply(ham, a, b, coeffs, s, V, W, work)
+    k0.record()
+    P.polfed_filter_apply(ham, a, b, coeffs, s, V, W, work)
+    k1.record()
+    torch.cuda.synchronize()
+    apply_ms = k0.elapsed_time(k1)
+    gbs = by / (launch_ms * 1e-3) / 1e9
+    return {"workload": WORKLOAD_NAMES[config], "format": fmt_name, "N": n, "nnz": nnz, "s": s,
+            "bytes_per_fused_launch": by, "launch_ms": launch_ms, "launches_timed": n_l,
+            "algorithmic_gbs": gbs, "frac_of_measured": gbs / peak,
+            "frac_of_nominal_8TBps": gbs / NOMINAL_HBM_GBS,
+            "filter_order": K, "filter_apply_ms": apply_ms,
+            "filter_steps_per_s": K / (apply_ms * 1e-3),
+            "us_per_product_in_filter": apply_ms * 1e3 / K,
+            "l2": "inputs exceed L2" if by > 4 * 126e6 else "working set fits L2 (not flushed)"}
 
 
 def time_to_nev(P, config: int):
@@ -425,7 +518,9 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--order", type=int, default=64, help="filter order K per step")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--format", default="auto", choices=["auto", "csr", "sell", "tiled", "flip"],
+    ap.add_argument("--per-config", default="1,2,3,4",
+                    help="other configs whose fused launch is timed at N=1 ('' to skip)")
+    ap.add_argument("--format", default="auto", choices=["auto", "csr", "sell", "tiled", "flip", "sector"],
                     help="auto: tiled where supported and n_sites >= 24, flip for full-space XX models, "
                          "else CSR")
     ap.add_argument("--no-cpu-baseline", action="store_true")
