@@ -82,6 +82,14 @@ bool sell_supports(const polfed_ham* ham, int s, const void* X, const void* Z, c
 int sell_step(const polfed_ham* ham, int s, double p, double q, double r, double c, const double* X,
               const double* Z, const double* V, double* Y, cudaStream_t st);
 
+// small_filter.cu: the whole recurrence in one persistent single-CTA kernel (n * s <= 4096).
+// small_filter_apply returns POLFED_ERANGE when the rows do not fit its shared memory.
+bool small_filter_supports(const polfed_ham* ham, int s);
+int csr_max_row_len(long long n, const int32_t* d_row_ptr, int* out);
+int small_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,
+                       int s, const double* d_V, double* d_W, double* cur, double* old,
+                       cudaStream_t st);
+
 // spmm_clenshaw.cu: the fused step without argument validation (flip handles: flip_step, SELL
 // handles: sell_step).
 int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
@@ -115,6 +123,7 @@ struct polfed_ham {
   const double* d_val = nullptr;
   bool owns = false;  // arrays allocated by polfed_build_hamiltonian
   int sm_count = 148;
+  int max_row_len = 0;   // longest CSR row (small_filter.cu)
   polfed::TiledPlan* tiled = nullptr;  // POLFED_FORMAT_TILED only (owned)
   polfed::FlipPlan* flip = nullptr;    // POLFED_FORMAT_FLIP only (owned)
   polfed::SellPlan* sell = nullptr;    // POLFED_FORMAT_SELL only (owned)

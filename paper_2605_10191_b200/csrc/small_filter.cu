@@ -1,0 +1,219 @@
+// The whole Clenshaw recurrence of Eq. (51) PAPER.md:427-431 in ONE persistent kernel for tiny
+// matrices (BASELINE config 1: n * s <= 4096; a fused launch moves 0.02 us of memory traffic
+// against 5 us of launch latency; SURVEY section 7 "tiny configs are latency-bound").  One CTA
+// keeps both auxiliary blocks in shared memory for all K steps: every thread owns a few
+// (row, column) items and keeps its own entries of b_{k+1}, b_{k+2} and V in registers, the CSR
+// entries of its rows are staged in shared memory once per launch, a CTA barrier separates the
+// steps and the blocks rotate by a pointer swap inside the kernel (Fig. 5).  The coefficients
+// travel as kernel parameters, up to kSmallChunk recurrence steps per launch, so nothing is
+// allocated and no device buffer beyond the caller's two-block workspace is needed.
+// (A cooperative multi-CTA variant with a grid barrier per step was measured on config 2 and
+// lost to single launches: 9.8 against 6.1 us per product.)
+#include <algorithm>
+
+#include "common.cuh"
+
+namespace polfed {
+namespace {
+
+constexpr int kSmallChunk = 384;  // recurrence steps per launch (3 KB of kernel parameters)
+
+struct SmallArgs {
+  int n, s, n_steps;
+  const int32_t* row_ptr;
+  const int32_t* col;
+  const double* val;
+  const double* V;
+  double* cur;  // b_{k+1}
+  double* old;  // b_{k+2}, overwritten by b_k
+  double* W;    // target of the final step (k = 0), if it is in this launch
+  double a, b;
+  int max_len;      // longest row of the matrix (entries staged per row slot)
+  int first_has_z;  // the first step of the whole recurrence has no b_{k+2}
+  int last_is_w;    // the last step of this launch is k = 0: factor 1, written to W
+  double c[kSmallChunk];  // c[i]: coefficient of step i of this launch
+};
+
+constexpr int kSingleItems = 4096;    // single-CTA variant: both blocks in shared memory
+constexpr int kSingleThreads = 1024;  // up to 4 items per thread
+
+// Every thread owns the items it = tid + j * n_threads for the whole recurrence, so its own
+// entries of b_{k+1}, b_{k+2} and V stay in registers, and the CSR entries of its rows are staged
+// once per launch in shared memory ([entry][row slot]: the s threads of a row share a slot).  Per
+// step it gathers b_{k+1} at its row's columns from shared memory and publishes b_k there.
+template <int J>
+__global__ void __launch_bounds__(kSingleThreads) small_filter_kernel(const SmallArgs a) {
+  constexpr bool SINGLE = true;
+  extern __shared__ double s_dyn[];
+  const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+  const int n_threads = gridDim.x * blockDim.x;
+  const int items = a.n * a.s;
+  const int rows_per_j = blockDim.x / a.s, slots = J * rows_per_j;
+  double* s_blocks = s_dyn;                                      // SINGLE: two blocks
+  double* ent_val = s_dyn + (SINGLE ? 2 * items : 0);            // [max_len][slots]
+  int* ent_col = reinterpret_cast<int*>(ent_val + a.max_len * slots);
+  double x_own[J], z_own[J], v_own[J];
+  int len[J], col_j[J];
+#pragma unroll
+  for (int j = 0; j < J; ++j) {
+    const int it = tid + j * n_threads;
+    x_own[j] = z_own[j] = v_own[j] = 0.0;
+    len[j] = col_j[j] = 0;
+    if (it < items) {
+      const int row = it / a.s;
+      col_j[j] = it - row * a.s;
+      const int e0 = __ldg(a.row_ptr + row);
+      len[j] = __ldg(a.row_ptr + row + 1) - e0;
+      const int slot = j * rows_per_j + threadIdx.x / a.s;
+      for (int k = col_j[j]; k < len[j]; k += a.s) {  // the row's threads share the copy
+        ent_val[k * slots + slot] = __ldg(a.val + e0 + k);
+        ent_col[k * slots + slot] = __ldg(a.col + e0 + k) * a.s;
+      }
+      x_own[j] = __ldcg(a.cur + it);
+      if (a.first_has_z) z_own[j] = __ldcg(a.old + it);
+      v_own[j] = __ldg(a.V + it);
+    }
+  }
+  double* cur = a.cur;
+  double* old = a.old;
+  if (SINGLE) {
+    cur = s_blocks;
+    old = s_blocks + items;
+#pragma unroll
+    for (int j = 0; j < J; ++j)
+      if (tid + j * n_threads < items) cur[tid + j * n_threads] = x_own[j];
+  }
+  __syncthreads();
+  const double p2 = 2.0 / a.b, q2 = -2.0 * a.a / a.b;
+  const int slot0 = threadIdx.x / a.s;
+  for (int i = 0; i < a.n_steps; ++i) {
+    const bool last = a.last_is_w && i + 1 == a.n_steps;
+    const double p = last ? 0.5 * p2 : p2, q = last ? 0.5 * q2 : q2;
+    const double r = (i == 0 && !a.first_has_z) ? 0.0 : -1.0;
+    const double c = a.c[i];
+    double* out = last ? a.W : old;
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const int it = tid + j * n_threads;
+      const double* ev = ent_val + j * rows_per_j + slot0;
+      const int* ec = ent_col + j * rows_per_j + slot0;
+      const double* xc = cur + col_j[j];
+      double acc = 0.0;
+#pragma unroll 4
+      for (int k = 0; k < len[j]; ++k)
+        acc = fma(ev[k * slots], SINGLE ? xc[ec[k * slots]] : __ldcg(xc + ec[k * slots]), acc);
+      if (it < items) {
+        double y = fma(p, acc, q * x_own[j]);
+        y = fma(r, z_own[j], y);
+        y = fma(c, v_own[j], y);
+        if (SINGLE && !last) out[it] = y;
+        else __stcg(out + it, y);
+        z_own[j] = x_own[j];
+        x_own[j] = y;
+      }
+    }
+    double* t = cur;  // "Permutation" of Fig. 5
+    cur = old;
+    old = t;
+    if (i + 1 < a.n_steps) {
+      __syncthreads();
+    }
+  }
+  if (SINGLE && !a.last_is_w) {
+    // more launches follow: publish b_{k+1} (cur) and b_{k+2} (old) in the caller's blocks, in the
+    // places the host expects after n_steps rotations
+    double* g_cur = (a.n_steps & 1) ? a.old : a.cur;
+    double* g_old = (a.n_steps & 1) ? a.cur : a.old;
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const int it = tid + j * n_threads;
+      if (it < items) {
+        g_cur[it] = x_own[j];
+        g_old[it] = z_own[j];
+      }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256) max_row_len_kernel(long long n, const int32_t* __restrict__ rp,
+                                                          int* out) {
+  const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int v = r < n ? rp[r + 1] - rp[r] : 0;
+  v = __reduce_max_sync(0xffffffffu, v);
+  if ((threadIdx.x & 31) == 0) atomicMax(out, v);
+}
+
+const void* const kKernels[4] = {
+    (const void*)small_filter_kernel<1>, (const void*)small_filter_kernel<2>,
+    (const void*)small_filter_kernel<4>, (const void*)small_filter_kernel<8>};
+
+}  // namespace
+
+// True when the persistent kernel takes the recurrence of this handle and block size.
+bool small_filter_supports(const polfed_ham* ham, int s) {
+  if (!ham || ham->tiled || ham->flip || ham->sell || ham->max_row_len < 1) return false;
+  return ham->n * (long long)s <= kSingleItems;
+}
+
+// Longest row of a CSR matrix (polfed_ham_from_csr records it in the handle).  Synchronises.
+int csr_max_row_len(long long n, const int32_t* d_row_ptr, int* out) {
+  *out = 0;
+  if (n < 1) return POLFED_OK;
+  int* d_max = nullptr;
+  POLFED_CUDA(cudaMalloc(&d_max, sizeof(int)));
+  cudaMemset(d_max, 0, sizeof(int));
+  max_row_len_kernel<<<(unsigned)((n + 255) / 256), 256>>>(n, d_row_ptr, d_max);
+  cudaError_t e = cudaMemcpy(out, d_max, sizeof(int), cudaMemcpyDeviceToHost);
+  cudaFree(d_max);
+  if (e != cudaSuccess) return fail(POLFED_ECUDA, "csr_max_row_len: %s", cudaGetErrorString(e));
+  return POLFED_OK;
+}
+
+// cur = c_K V has been written by the caller; runs steps k = K-1 .. 0.
+int small_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const double* c, int s,
+                       const double* d_V, double* d_W, double* cur, double* old, cudaStream_t st) {
+  constexpr int kSmemCap = 200 * 1024;
+  static bool configured = false;
+  if (!configured) {
+    for (int v = 0; v < 4; ++v)
+      POLFED_CUDA(cudaFuncSetAttribute(kKernels[v], cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       kSmemCap));
+    configured = true;
+  }
+  const int items = (int)ham->n * s;
+  const int j_used = (items + kSingleThreads - 1) / kSingleThreads;
+  int jlog = 0;  // items per thread of the instantiation: 1, 2, 4 or 8
+  while ((1 << jlog) < j_used) ++jlog;
+  const size_t smem = 2 * (size_t)items * sizeof(double) +
+                      ((size_t)1 << jlog) * (kSingleThreads / s) * ham->max_row_len * 12 + 16;
+  if (jlog > 3 || smem > (size_t)kSmemCap) return POLFED_ERANGE;  // caller: single launches
+  const void* kernel = kKernels[jlog];
+
+  SmallArgs args{};
+  args.n = (int)ham->n;
+  args.s = s;
+  args.row_ptr = ham->d_row_ptr;
+  args.col = ham->d_col;
+  args.val = ham->d_val;
+  args.V = d_V;
+  args.W = d_W;
+  args.a = a_;
+  args.b = b_;
+  args.max_len = ham->max_row_len;
+  for (int k = K - 1; k >= 0;) {  // launches of up to kSmallChunk steps, k descending
+    const int n_steps = std::min(k + 1, kSmallChunk);
+    args.n_steps = n_steps;
+    args.cur = cur;
+    args.old = old;
+    args.first_has_z = (k != K - 1);
+    args.last_is_w = (k - n_steps + 1 == 0);
+    for (int i = 0; i < n_steps; ++i) args.c[i] = c[k - i];
+    void* params[] = {&args};
+    POLFED_CUDA(cudaLaunchKernel(kernel, dim3(1), dim3(kSingleThreads), params, smem, st));
+    if (n_steps & 1) std::swap(cur, old);  // the kernel's rotation, seen from the host
+    k -= n_steps;
+  }
+  return POLFED_OK;
+}
+
+}  // namespace polfed

@@ -332,6 +332,10 @@ int polfed_filter_apply(const polfed_ham* ham, double a, double b, int K, const 
   double* old = cur + len;                     // b_{k+2}, overwritten by b_k
   int rc = polfed::scale_copy(len, d_V, cur, h_coeffs[K], ham->sm_count, st);  // b_K = c_K V
   if (rc) return rc;
+  if (polfed::small_filter_supports(ham, s)) {  // one persistent kernel for all K steps
+    rc = polfed::small_filter_apply(ham, a, b, K, h_coeffs, s, d_V, d_W, cur, old, st);
+    if (rc != POLFED_ERANGE) return rc;
+  }
   const double p2 = 2.0 / b, q2 = -2.0 * a / b;
   for (int k = K - 1; k >= 1; --k) {
     // b_k = 2 H~ b_{k+1} - b_{k+2} + c_k V; b_{K+1} = 0 is never read
