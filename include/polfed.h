@@ -274,6 +274,20 @@ int polfed_kpm_moments(const polfed_ham* ham, double a, double b, int n_moments,
 int polfed_kpm_dos(const double* h_moments, int n_moments, const double* e_rescaled, int n_points,
                    double* rho);
 
+/* The two tall-skinny products of the full reorthogonalisation (Eq. 9, 11 PAPER.md:147-153; cost
+ * O(M^2 D)), exported so that they can be tested and timed on their own:
+ *   polfed_block_gram:    C_j = Q_j^T B      for j < n_panels   (C: n_panels x s x s, row-major)
+ *   polfed_block_update:  B = beta B + alpha sum_j Q_j C_j
+ * Q_j = d_Q + j * panel_stride doubles, each n x s row-major like B; s in {1,2,4,8,16,32}; all
+ * pointers DEVICE, 16-byte aligned.  Every sum runs in a fixed order (bit-reproducible).
+ * variant: 0 = the library's choice (fp64 tensor-core mma for s >= 8), 1 = the shared-memory FMA
+ * kernel, 2 = tensor cores (s >= 8 only, else the FMA kernel).  Enqueued on `stream`; scratch for
+ * the per-CTA partial sums comes from the device's stream-ordered pool. */
+int polfed_block_gram(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
+                      const double* d_B, double* d_C, int variant, void* stream);
+int polfed_block_update(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
+                        const double* d_C, double alpha, double beta, double* d_B, void* stream);
+
 typedef struct {
   double tol;             /* absolute bound on ||H x - lambda x||; <= 0: 1e-8 * max(|E_min|,|E_max|) */
   int32_t max_krylov_dim; /* <= 0: 5 nev + 8 s rounded up to a multiple of s (R10), capped by n and by free memory */

@@ -29,6 +29,7 @@ EXPORTS = (
     "polfed_filter_apply_host", "polfed_filter_coeffs",
     "polfed_spectrum_bounds", "polfed_block_lanczos_eigs",
     "polfed_kpm_workspace_bytes", "polfed_kpm_moments", "polfed_kpm_dos",
+    "polfed_block_gram", "polfed_block_update",
 )
 
 
@@ -110,6 +111,8 @@ def lib() -> C.CDLL:
     L.polfed_kpm_workspace_bytes.argtypes = [i64, i32, i32]
     L.polfed_kpm_moments.argtypes = [p, f64, f64, i32, i32, p, p, p, p]
     L.polfed_kpm_dos.argtypes = [p, i32, p, i32, p]
+    L.polfed_block_gram.argtypes = [i32, i64, p, i32, i64, p, p, i32, p]
+    L.polfed_block_update.argtypes = [i32, i64, p, i32, i64, p, f64, f64, p, p]
     _lib = L
     return L
 
@@ -366,6 +369,24 @@ def polfed_spectrum_bounds(ham: Ham, v0, n_steps: int = 0, margin: float = -1.0,
     _check(lib().polfed_spectrum_bounds(C.c_void_p(ham.handle), n_steps, _dev(v0), margin,
                                         _stream(stream), *[C.byref(o) for o in out]))
     return tuple(o.value for o in out)
+
+
+def polfed_block_gram(Q, B, variant: int = 0, stream=None):
+    """C[j] = Q[j]^T B for the panels Q[j] (CUDA tensor k x n x s) and the block B (n x s):
+    returns a CUDA tensor k x s x s.  variant: 0 library's choice, 1 FMA kernel, 2 tensor cores."""
+    import torch
+    k, n, s = Q.shape
+    Cm = torch.empty(k, s, s, dtype=torch.float64, device="cuda")
+    _check(lib().polfed_block_gram(s, n, _dev(Q), k, n * s, _block(B, n, s), _dev(Cm), variant,
+                                   _stream(stream)))
+    return Cm
+
+
+def polfed_block_update(Q, Cm, B, alpha: float, beta: float, stream=None) -> None:
+    """B = beta B + alpha sum_j Q[j] C[j] in place (Q: k x n x s, C: k x s x s, B: n x s)."""
+    k, n, s = Q.shape
+    _check(lib().polfed_block_update(s, n, _dev(Q), k, n * s, _dev(Cm), alpha, beta,
+                                     _block(B, n, s), _stream(stream)))
 
 
 def polfed_kpm_workspace_bytes(n: int, s: int, n_moments: int) -> int:

@@ -98,6 +98,8 @@ int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, do
 // tallskinny.cu (see there).  d_C is zeroed by ts_gram before accumulation.
 int ts_gram(int s, long long n, const double* Q, int n_panels, size_t stride, const double* B,
             double* d_C, int sm_count, cudaStream_t st);
+int ts_gram_variant(int s, long long n, const double* Q, int n_panels, size_t stride, const double* B,
+                    double* d_C, int sm_count, int variant, cudaStream_t st);
 int ts_update(int s, long long n, const double* Q, int n_panels, size_t stride, const double* d_C,
               double alpha, double beta, double* B, cudaStream_t st);
 int ts_residual_norms(int s, long long n, const double* A, const double* B, const double* d_e,

@@ -3,9 +3,12 @@
 //   update  B = beta B + alpha Q C     W -= Q (Q^T W), Ritz back-map u = V t (Eq. 43), W R^-1
 // PAPER.md:136-172 (Eq. 8-14), 364-382.  Q is "panel-blocked": n_panels blocks of n x S
 // row-major, panel j at Q + j*panel_stride; B is one n x S block; C is (n_panels*S) x S
-// row-major.  Both kernels stream Q exactly once; they are bandwidth-bound like the filter,
-// but run once per block step against K filter launches, so they are written for clarity
-// (shared-memory tiles, register accumulators, one fp64 atomicAdd per output per CTA).
+// row-major.  Both kernels stream Q exactly once.  Every reduction is in a fixed order (per-CTA
+// partial results, then one pass that adds them by ascending CTA index), so H_L, the CholeskyQR
+// factors and with them the iteration count of the eigen-solver are reproducible run to run.
+// For s in {8, 16, 32} the Gram product runs on the fp64 tensor cores (mma.sync m8n8k4, operands
+// straight from global memory into fragments); the shared-memory FMA kernel serves s < 8 and is
+// the measured alternative (profiles/r02_reorth.md).
 #include "common.cuh"
 
 namespace polfed {
@@ -18,7 +21,7 @@ constexpr int kTileRows = 32;
 template <int S>
 __global__ void __launch_bounds__(kTsThreads)
 gram_kernel(long long n, const double* __restrict__ Q, size_t panel_stride,
-            const double* __restrict__ B, double* __restrict__ C) {
+            const double* __restrict__ B, double* __restrict__ partial) {
   constexpr int OUT = S * S;
   constexpr int PER = (OUT + kTsThreads - 1) / kTsThreads;  // outputs per thread
   __shared__ double As[kTileRows][S];
@@ -55,8 +58,96 @@ gram_kernel(long long n, const double* __restrict__ Q, size_t panel_stride,
 #pragma unroll
   for (int t = 0; t < PER; ++t) {
     const int o = threadIdx.x + t * kTsThreads;
-    if (o < OUT) atomicAdd(C + (size_t)j * OUT + o, acc[t]);
+    if (o < OUT) partial[((size_t)blockIdx.x * gridDim.y + j) * OUT + o] = acc[t];
   }
+}
+
+// ---- the same product on the fp64 tensor cores ------------------------------------------------
+// mma.sync.aligned.m8n8k4 (D = A B + C, A 8x4 row-major, B 4x8 column-major): lane l holds
+// A[l/4][l%4], B[l%4][l/4] and C[l/4][2(l%4) + {0,1}].  With A = Q_j^T and B = B over four rows r,
+// both fragments are element (r0 + l%4, tile * 8 + l/4) of their row-major blocks, so a warp
+// instruction reads four 64-byte row pieces.  A warp owns all (S/8)^2 output tiles and walks
+// over rows; the CTA adds its warps in warp order.
+__device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(d0), "+d"(d1)
+               : "d"(a), "d"(b));
+}
+
+constexpr int kDmmaThreads = 128;
+
+template <int S>
+__global__ void __launch_bounds__(kDmmaThreads)
+gram_dmma_kernel(long long n, const double* __restrict__ Q, size_t panel_stride,
+                 const double* __restrict__ B, double* __restrict__ partial) {
+  constexpr int T = S / 8, OUT = S * S, WARPS = kDmmaThreads / 32;
+  __shared__ double red[WARPS][OUT];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int j = blockIdx.y;
+  const double* Qj = Q + (size_t)j * panel_stride + (lane & 3) * S + (lane >> 2);
+  const double* Bl = B + (lane & 3) * S + (lane >> 2);
+  double acc[T][T][2];
+#pragma unroll
+  for (int m = 0; m < T; ++m)
+#pragma unroll
+    for (int c = 0; c < T; ++c) acc[m][c][0] = acc[m][c][1] = 0.0;
+  // rows in groups of 4; group g -> warp (g mod all warps of this panel), ascending
+  const long long groups = n / 4;
+  const long long stride = (long long)gridDim.x * WARPS;
+  for (long long g = (long long)blockIdx.x * WARPS + warp; g < groups; g += stride) {
+    const size_t at = (size_t)g * 4 * S;
+    double a[T], b[T];
+#pragma unroll
+    for (int m = 0; m < T; ++m) {
+      a[m] = __ldg(Qj + at + m * 8);
+      b[m] = __ldg(Bl + at + m * 8);
+    }
+#pragma unroll
+    for (int m = 0; m < T; ++m)
+#pragma unroll
+      for (int c = 0; c < T; ++c) dmma(acc[m][c][0], acc[m][c][1], a[m], b[c]);
+  }
+  // the last n mod 4 rows: warp 0 of CTA 0, lanes of the missing rows feed zeros
+  if (blockIdx.x == 0 && warp == 0 && groups * 4 < n) {
+    const size_t at = (size_t)groups * 4 * S;
+    const bool ok = groups * 4 + (lane & 3) < n;
+    double a[T], b[T];
+#pragma unroll
+    for (int m = 0; m < T; ++m) {
+      a[m] = ok ? __ldg(Qj + at + m * 8) : 0.0;
+      b[m] = ok ? __ldg(Bl + at + m * 8) : 0.0;
+    }
+#pragma unroll
+    for (int m = 0; m < T; ++m)
+#pragma unroll
+      for (int c = 0; c < T; ++c) dmma(acc[m][c][0], acc[m][c][1], a[m], b[c]);
+  }
+#pragma unroll
+  for (int m = 0; m < T; ++m)
+#pragma unroll
+    for (int c = 0; c < T; ++c) {
+      const int row = m * 8 + (lane >> 2), col = c * 8 + 2 * (lane & 3);
+      red[warp][row * S + col] = acc[m][c][0];
+      red[warp][row * S + col + 1] = acc[m][c][1];
+    }
+  __syncthreads();
+  for (int o = threadIdx.x; o < OUT; o += kDmmaThreads) {
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) t += red[w][o];
+    partial[((size_t)blockIdx.x * gridDim.y + j) * OUT + o] = t;
+  }
+}
+
+// out[i] = sum over p = 0..count-1 (ascending) of partial[p * len + i]
+__global__ void __launch_bounds__(256) sum_partials_kernel(int count, size_t len,
+                                                           const double* __restrict__ partial,
+                                                           double* __restrict__ out) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= len) return;
+  double t = 0.0;
+  for (int p = 0; p < count; ++p) t += partial[(size_t)p * len + i];
+  out[i] = t;
 }
 
 // ---- B = beta B + alpha sum_j Q_j C_j on one tile of rows per CTA -----------------------------
@@ -101,6 +192,64 @@ update_kernel(long long n, const double* Q, int n_panels, size_t panel_stride,
   }
 }
 
+// ---- the same update on the fp64 tensor cores --------------------------------------------------
+// D (8 rows x 8 columns) += Q_j[8 rows][4 columns k0..k0+3] C_j[k0..k0+3][8 columns]: the A fragment
+// of lane l is Q_j[r0 + l/4][k0 + l%4], the B fragment C_j[k0 + l%4][8c + l/4].  A warp owns
+// kUpdGroups groups of 8 rows, so every C fragment (read through L1) feeds kUpdGroups mma.
+constexpr int kUpdGroups = 4;
+
+template <int S>
+__global__ void __launch_bounds__(kDmmaThreads)
+update_dmma_kernel(long long n, const double* __restrict__ Q, int n_panels, size_t panel_stride,
+                   const double* __restrict__ C, double alpha, double beta, double* B) {
+  constexpr int T = S / 8;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long base = ((long long)blockIdx.x * (kDmmaThreads / 32) + warp) * (8 * kUpdGroups);
+  if (base >= n) return;
+  double acc[kUpdGroups][T][2];
+#pragma unroll
+  for (int g = 0; g < kUpdGroups; ++g)
+#pragma unroll
+    for (int c = 0; c < T; ++c) acc[g][c][0] = acc[g][c][1] = 0.0;
+  long long row[kUpdGroups];
+#pragma unroll
+  for (int g = 0; g < kUpdGroups; ++g) row[g] = base + g * 8 + (lane >> 2);
+  for (int j = 0; j < n_panels; ++j) {
+    const double* Qj = Q + (size_t)j * panel_stride + (lane & 3);
+    const double* Cj = C + (size_t)j * S * S + (lane & 3) * S + (lane >> 2);
+#pragma unroll 2
+    for (int k0 = 0; k0 < S; k0 += 4) {
+      double a[kUpdGroups], cf[T];
+#pragma unroll
+      for (int g = 0; g < kUpdGroups; ++g)
+        a[g] = row[g] < n ? __ldg(Qj + (size_t)row[g] * S + k0) : 0.0;
+#pragma unroll
+      for (int c = 0; c < T; ++c) cf[c] = __ldg(Cj + k0 * S + c * 8);
+#pragma unroll
+      for (int g = 0; g < kUpdGroups; ++g)
+#pragma unroll
+        for (int c = 0; c < T; ++c) dmma(acc[g][c][0], acc[g][c][1], a[g], cf[c]);
+    }
+  }
+#pragma unroll
+  for (int g = 0; g < kUpdGroups; ++g) {
+    if (row[g] >= n) continue;
+#pragma unroll
+    for (int c = 0; c < T; ++c) {
+      double2* out = reinterpret_cast<double2*>(B + (size_t)row[g] * S + c * 8 + 2 * (lane & 3));
+      double2 o = make_double2(0.0, 0.0);
+      if (beta != 0.0) {
+        o = *out;
+        o.x *= beta;
+        o.y *= beta;
+      }
+      o.x = fma(alpha, acc[g][c][0], o.x);
+      o.y = fma(alpha, acc[g][c][1], o.y);
+      *out = o;
+    }
+  }
+}
+
 // ---- per-column sum of squares of (A - B diag(e)) ----------------------------------------------
 template <int S>
 __global__ void __launch_bounds__(kTsThreads)
@@ -119,7 +268,7 @@ residual_norm_kernel(long long n, const double* __restrict__ A, const double* __
   __syncthreads();
   if (g == 0) {
     for (int k = 1; k < GROUPS; ++k) sum += red[k * S + b];
-    atomicAdd(out + b, sum);
+    out[(size_t)blockIdx.x * S + b] = sum;  // per-CTA partial, added up in CTA order afterwards
   }
 }
 
@@ -161,28 +310,74 @@ __global__ void __launch_bounds__(256) moments_kernel(long long n, const int32_t
     }
     __syncthreads();
   }
-  if (threadIdx.x == 0) {
-    atomicAdd(out, red[0][0]);
-    atomicAdd(out + 1, red[1][0]);
+  if (threadIdx.x == 0) {  // per-CTA partials, added up in CTA order afterwards
+    out[2 * blockIdx.x] = red[0][0];
+    out[2 * blockIdx.x + 1] = red[1][0];
   }
 }
 
+// Scratch for per-CTA partial results from the stream-ordered pool (reused after the first call).
+struct PoolBuf {
+  double* p = nullptr;
+  cudaStream_t st;
+  explicit PoolBuf(cudaStream_t s) : st(s) {}
+  cudaError_t alloc(size_t doubles) {
+    return cudaMallocAsync(reinterpret_cast<void**>(&p), sizeof(double) * (doubles ? doubles : 1), st);
+  }
+  ~PoolBuf() {
+    if (p) cudaFreeAsync(p, st);
+  }
+};
+
+int sum_partials(int count, size_t len, const double* partial, double* out, cudaStream_t st) {
+  sum_partials_kernel<<<(unsigned)((len + 255) / 256), 256, 0, st>>>(count, len, partial, out);
+  POLFED_LAUNCH_CHECK("sum_partials_kernel");
+  return POLFED_OK;
+}
+
+// variant: 0 = automatic (tensor cores for S >= 8), 1 = shared-memory FMA kernel, 2 = tensor cores
 template <int S>
 int gram_launch(long long n, const double* Q, int n_panels, size_t stride, const double* B, double* C,
-                int sm_count, cudaStream_t st) {
-  const long long n_tiles = (n + kTileRows - 1) / kTileRows;
-  long long gx = (long long)sm_count * 8 / (n_panels > 0 ? n_panels : 1);
-  if (gx < 1) gx = 1;
-  if (gx > n_tiles) gx = n_tiles;
+                int sm_count, int variant, cudaStream_t st) {
+  const bool dmma_ok = S >= 8;
+  const bool use_dmma = dmma_ok && variant != 1;
+  long long gx;
+  if (use_dmma) {
+    const long long groups = (n / 4 + kDmmaThreads / 32 - 1) / (kDmmaThreads / 32);
+    gx = (long long)sm_count * 8 / n_panels;
+    if (gx < 1) gx = 1;
+    if (gx > groups) gx = groups > 0 ? groups : 1;
+  } else {
+    const long long n_tiles = (n + kTileRows - 1) / kTileRows;
+    gx = (long long)sm_count * 8 / n_panels;
+    if (gx < 1) gx = 1;
+    if (gx > n_tiles) gx = n_tiles;
+  }
+  const size_t len = (size_t)n_panels * S * S;
+  PoolBuf partial(st);
+  POLFED_CUDA(partial.alloc((size_t)gx * len));
   dim3 grid((unsigned)gx, (unsigned)n_panels);
-  gram_kernel<S><<<grid, kTsThreads, 0, st>>>(n, Q, stride, B, C);
+  if constexpr (S >= 8) {
+    if (use_dmma) gram_dmma_kernel<S><<<grid, kDmmaThreads, 0, st>>>(n, Q, stride, B, partial.p);
+  }
+  if (!use_dmma) gram_kernel<S><<<grid, kTsThreads, 0, st>>>(n, Q, stride, B, partial.p);
   POLFED_LAUNCH_CHECK("gram_kernel");
-  return POLFED_OK;
+  return sum_partials((int)gx, len, partial.p, C, st);
 }
 
 template <int S>
 int update_launch(long long n, const double* Q, int n_panels, size_t stride, const double* C, double alpha,
                   double beta, double* B, cudaStream_t st) {
+  if constexpr (S >= 8) {  // tensor cores, unless B is one of the panels (in-place W R^-1): the
+                           // shared-memory kernel stages its rows before it writes them
+    if (n_panels > 0 && (B + (size_t)n * S <= Q || B >= Q + (size_t)(n_panels - 1) * stride + (size_t)n * S)) {
+      constexpr int ROWS_D = (kDmmaThreads / 32) * 8 * kUpdGroups;
+      update_dmma_kernel<S><<<(unsigned)((n + ROWS_D - 1) / ROWS_D), kDmmaThreads, 0, st>>>(
+          n, Q, n_panels, stride, C, alpha, beta, B);
+      POLFED_LAUNCH_CHECK("update_dmma_kernel");
+      return POLFED_OK;
+    }
+  }
   constexpr int GROUPS = kTsThreads / S;
   constexpr int ROWS = GROUPS * ((kTileRows + GROUPS - 1) / GROUPS);
   const unsigned grid = (unsigned)((n + ROWS - 1) / ROWS);
@@ -197,9 +392,11 @@ int resid_launch(long long n, const double* A, const double* B, const double* e,
   constexpr int GROUPS = kTsThreads / S;
   long long want = (n + GROUPS - 1) / GROUPS;
   const unsigned grid = (unsigned)(want < (long long)sm_count * 8 ? want : (long long)sm_count * 8);
-  residual_norm_kernel<S><<<grid, kTsThreads, 0, st>>>(n, A, B, e, out);
+  PoolBuf partial(st);
+  POLFED_CUDA(partial.alloc((size_t)grid * S));
+  residual_norm_kernel<S><<<grid, kTsThreads, 0, st>>>(n, A, B, e, partial.p);
   POLFED_LAUNCH_CHECK("residual_norm_kernel");
-  return POLFED_OK;
+  return sum_partials((int)grid, S, partial.p, out, st);
 }
 
 }  // namespace
@@ -215,12 +412,21 @@ int resid_launch(long long n, const double* A, const double* B, const double* e,
     default: return fail(POLFED_EINVAL, "block size s=%d not in {1,2,4,8,16,32}", s); \
   }
 
+constexpr int g_gram_variant = 0;
+
 int ts_gram(int s, long long n, const double* Q, int n_panels, size_t stride, const double* B, double* d_C,
             int sm_count, cudaStream_t st) {
   if (n_panels <= 0 || n <= 0) return POLFED_OK;
-  POLFED_CUDA(cudaMemsetAsync(d_C, 0, sizeof(double) * (size_t)n_panels * s * s, st));
-  POLFED_BY_S(s, (gram_launch<S_>(n, Q, n_panels, stride, B, d_C, sm_count, st)));
+  POLFED_BY_S(s, (gram_launch<S_>(n, Q, n_panels, stride, B, d_C, sm_count, g_gram_variant, st)));
 }
+
+int ts_gram_variant(int s, long long n, const double* Q, int n_panels, size_t stride, const double* B,
+                    double* d_C, int sm_count, int variant, cudaStream_t st) {
+  if (n_panels <= 0 || n <= 0) return POLFED_OK;
+  POLFED_BY_S(s, (gram_launch<S_>(n, Q, n_panels, stride, B, d_C, sm_count, variant, st)));
+}
+
+
 
 int ts_update(int s, long long n, const double* Q, int n_panels, size_t stride, const double* d_C,
               double alpha, double beta, double* B, cudaStream_t st) {
@@ -230,8 +436,10 @@ int ts_update(int s, long long n, const double* Q, int n_panels, size_t stride, 
 
 int ts_residual_norms(int s, long long n, const double* A, const double* B, const double* d_e, double* d_out,
                       int sm_count, cudaStream_t st) {
-  POLFED_CUDA(cudaMemsetAsync(d_out, 0, sizeof(double) * (size_t)s, st));
-  if (n <= 0) return POLFED_OK;
+  if (n <= 0) {
+    POLFED_CUDA(cudaMemsetAsync(d_out, 0, sizeof(double) * (size_t)s, st));
+    return POLFED_OK;
+  }
   POLFED_BY_S(s, (resid_launch<S_>(n, A, B, d_e, d_out, sm_count, st)));
 }
 
@@ -244,11 +452,47 @@ int ts_gather_columns(long long n, const double* src, int src_ld, const int* d_c
 }
 
 int csr_moments(const polfed_ham* ham, double* d_out2, cudaStream_t st) {
-  POLFED_CUDA(cudaMemsetAsync(d_out2, 0, 2 * sizeof(double), st));
-  if (ham->n == 0) return POLFED_OK;
-  moments_kernel<<<ham->sm_count * 8, 256, 0, st>>>(ham->n, ham->d_row_ptr, ham->d_col, ham->d_val, d_out2);
+  if (ham->n == 0) {
+    POLFED_CUDA(cudaMemsetAsync(d_out2, 0, 2 * sizeof(double), st));
+    return POLFED_OK;
+  }
+  const int grid = ham->sm_count * 8;
+  PoolBuf partial(st);
+  POLFED_CUDA(partial.alloc((size_t)grid * 2));
+  moments_kernel<<<grid, 256, 0, st>>>(ham->n, ham->d_row_ptr, ham->d_col, ham->d_val, partial.p);
   POLFED_LAUNCH_CHECK("moments_kernel");
-  return POLFED_OK;
+  return sum_partials(grid, 2, partial.p, d_out2, st);
 }
 
 }  // namespace polfed
+
+using polfed::fail;
+
+extern "C" {
+
+int polfed_block_gram(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
+                      const double* d_B, double* d_C, int variant, void* stream) {
+  if (!polfed::valid_block_size(s)) return fail(POLFED_EINVAL, "polfed_block_gram: bad block size s=%d", s);
+  if (n < 0 || n_panels < 0 || panel_stride < 0 || variant < 0 || variant > 2)
+    return fail(POLFED_EINVAL, "polfed_block_gram: bad argument");
+  if (n == 0 || n_panels == 0) return POLFED_OK;
+  if (!d_Q || !d_B || !d_C || !polfed::aligned16(d_Q) || !polfed::aligned16(d_B))
+    return fail(POLFED_EINVAL, "polfed_block_gram: NULL or misaligned block");
+  int dev = 0, sms = 148;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  return polfed::ts_gram_variant(s, n, d_Q, n_panels, (size_t)panel_stride, d_B, d_C, sms, variant,
+                                 static_cast<cudaStream_t>(stream));
+}
+
+int polfed_block_update(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
+                        const double* d_C, double alpha, double beta, double* d_B, void* stream) {
+  if (!polfed::valid_block_size(s)) return fail(POLFED_EINVAL, "polfed_block_update: bad block size s=%d", s);
+  if (n < 0 || n_panels < 0 || panel_stride < 0) return fail(POLFED_EINVAL, "polfed_block_update: bad argument");
+  if (n == 0) return POLFED_OK;
+  if (!d_B || (n_panels > 0 && (!d_Q || !d_C)))
+    return fail(POLFED_EINVAL, "polfed_block_update: NULL block");
+  return polfed::ts_update(s, n, d_Q, n_panels, (size_t)panel_stride, d_C, alpha, beta, d_B,
+                           static_cast<cudaStream_t>(stream));
+}
+
+}  // extern "C"
