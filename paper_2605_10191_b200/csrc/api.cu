@@ -2,6 +2,7 @@
 #include <new>
 
 #include "common.cuh"
+#include "packed.cuh"
 
 namespace polfed {
 
@@ -67,6 +68,13 @@ int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const 
       return rc;
     }
   }
+  {  // the packed form of the same matrix, when its off-diagonal values are few (packed.cuh)
+    int rc = polfed::build_packed_plan(h, nullptr, &h->packed);
+    if (rc) {
+      delete h;
+      return rc;
+    }
+  }
   *out = h;
   return POLFED_OK;
 }
@@ -76,6 +84,7 @@ int polfed_ham_destroy(polfed_ham* ham) {
   polfed::destroy_tiled_plan(ham->tiled);
   polfed::destroy_flip_plan(ham->flip);
   polfed::destroy_sell_plan(ham->sell);
+  polfed::destroy_packed_plan(ham->packed);
   if (ham->owns) {
     cudaFree(const_cast<int32_t*>(ham->d_row_ptr));
     cudaFree(const_cast<int32_t*>(ham->d_col));

@@ -52,6 +52,7 @@ struct DevTerm {
 struct TiledPlan;  // tiled.cuh
 struct FlipPlan;   // flip.cuh
 struct SellPlan;   // sell.cuh
+struct PackedPlan; // packed.cuh
 
 // assemble.cu: CSR of a term list over a basis; arrays cudaMalloc'ed, owned by the caller.
 int assemble_csr(const polfed_basis* basis, const std::vector<DevTerm>& terms, int dot_bits,
@@ -129,4 +130,5 @@ struct polfed_ham {
   polfed::TiledPlan* tiled = nullptr;  // POLFED_FORMAT_TILED only (owned)
   polfed::FlipPlan* flip = nullptr;    // POLFED_FORMAT_FLIP only (owned)
   polfed::SellPlan* sell = nullptr;    // POLFED_FORMAT_SELL only (owned)
+  polfed::PackedPlan* packed = nullptr;  // every handle whose matrix qualifies (owned)
 };

@@ -13,6 +13,7 @@
 // across the lane group, and handed round by shuffles.  The epilogue reads Z and V and
 // writes Y in the same pass -- there is no separate axpy kernel.
 #include "common.cuh"
+#include "packed.cuh"
 
 namespace polfed {
 namespace {
@@ -83,12 +84,25 @@ __device__ __forceinline__ void store_stream(double* p, const Acc<VEC>& a) {
   }
 }
 
-template <int S, int VEC_, bool USE_Z, bool USE_V>
+// NV > 0 (PACKED): row_ptr/col are those of the packed plan (col = column | value class << 28, off-diagonal
+// entries only), val is the dense diagonal and vt the value table (packed.cuh).
+// Value of class `cls` out of NV table entries: NV = 1 a constant, NV = 2 a register select.
+template <int NV>
+__device__ __forceinline__ double pick_val(unsigned cls, const PackedVals& vt) {
+  if constexpr (NV == 1) {
+    return vt.v[0];
+  } else {
+    return cls ? vt.v[1] : vt.v[0];
+  }
+}
+
+template <int S, int VEC_, bool USE_Z, bool USE_V, int NV>
 __global__ void __launch_bounds__(kThreads)
 fused_step_kernel(int n, const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ col,
                   const double* __restrict__ val, const double* __restrict__ X, const double* Z,
                   const double* V, double* Y, double p, double q, double r, double c,
-                  int rows_per_cta) {
+                  int rows_per_cta, const PackedVals vt) {
+  constexpr bool PACKED = NV > 0;
   using Sh = Shape<S, VEC_>;
   constexpr int VEC = Sh::VEC, LPR = Sh::LPR, RPW = Sh::RPW;
   const int lane = threadIdx.x & 31;
@@ -113,8 +127,14 @@ fused_step_kernel(int n, const int32_t* __restrict__ row_ptr, const int32_t* __r
     if constexpr (LPR == 1) {
       // one thread per row (S = 1, 2)
       for (int e = e0; e < e1; ++e) {
-        const int cj = __ldcs(col + e);
-        const double vj = __ldcs(val + e);
+        int cj = __ldcs(col + e);
+        double vj;
+        if constexpr (PACKED) {
+          vj = pick_val<NV>((unsigned)cj >> 28, vt);
+          cj &= 0x0fffffff;
+        } else {
+          vj = __ldcs(val + e);
+        }
         const Acc<VEC> x = load_gather<VEC>(X + (size_t)cj * S);
 #pragma unroll
         for (int t = 0; t < VEC; ++t) acc.v[t] = fma(vj, x.v[t], acc.v[t]);
@@ -128,13 +148,19 @@ fused_step_kernel(int n, const int32_t* __restrict__ row_ptr, const int32_t* __r
         double vv = 0.0;
         if (e < e1) {
           cc = __ldcs(col + e);
-          vv = __ldcs(val + e);
+          if constexpr (!PACKED) vv = __ldcs(val + e);
         }
         const int rem = len - off;  // entries of this row left in the chunk (may be <= 0)
 #pragma unroll
         for (int j = 0; j < LPR; ++j) {
-          const int cj = __shfl_sync(0xffffffffu, cc, j, LPR);
-          const double vj = __shfl_sync(0xffffffffu, vv, j, LPR);
+          int cj = __shfl_sync(0xffffffffu, cc, j, LPR);
+          double vj;
+          if constexpr (PACKED) {  // one shuffle per entry; the value is a table read
+            vj = pick_val<NV>((unsigned)cj >> 28, vt);
+            cj &= 0x0fffffff;
+          } else {
+            vj = __shfl_sync(0xffffffffu, vv, j, LPR);
+          }
           if (j < rem) {
             const Acc<VEC> x = load_gather<VEC>(X + (size_t)cj * S + sl * VEC);
 #pragma unroll
@@ -148,8 +174,10 @@ fused_step_kernel(int n, const int32_t* __restrict__ row_ptr, const int32_t* __r
       const size_t at = (size_t)row * S + sl * VEC;
       const Acc<VEC> xi = load_gather<VEC>(X + at);
       Acc<VEC> y;
+      double qd = q;
+      if constexpr (PACKED) qd = fma(p, __ldg(val + row), q);  // the dense diagonal
 #pragma unroll
-      for (int t = 0; t < VEC; ++t) y.v[t] = fma(p, acc.v[t], q * xi.v[t]);
+      for (int t = 0; t < VEC; ++t) y.v[t] = fma(p, acc.v[t], qd * xi.v[t]);
       if constexpr (USE_Z) {
         const Acc<VEC> z = load_stream<VEC>(Z + at);
 #pragma unroll
@@ -193,15 +221,27 @@ int launch_step_v(const polfed_ham* ham, double p, double q, double r, double c,
   const int rows_per_cta = rows_per_pass * passes;
   const unsigned grid = (unsigned)((n + (long long)rows_per_cta - 1) / rows_per_cta);
   const bool uz = (r != 0.0), uv = (c != 0.0);
-#define POLFED_GO(UZ, UV)                                                                      \
-  fused_step_kernel<S, VEC, UZ, UV><<<grid, kThreads, 0, st>>>(n, ham->d_row_ptr, ham->d_col,  \
-                                                          ham->d_val, X, Z, V, Y, p, q, r, c,  \
-                                                          rows_per_cta)
-  if (uz && uv) POLFED_GO(true, true);
-  else if (uz) POLFED_GO(true, false);
-  else if (uv) POLFED_GO(false, true);
-  else POLFED_GO(false, false);
+  PackedVals vt{};
+  const PackedPlan* pk = ham->packed;
+  if (pk)
+    for (int i = 0; i < 16; ++i) vt.v[i] = pk->vals[i];
+  const int nv = pk ? pk->n_vals : 0;
+#define POLFED_PK(UZ, UV, NV)                                                                    \
+  fused_step_kernel<S, VEC, UZ, UV, NV><<<grid, kThreads, 0, st>>>(                              \
+      n, pk->d_row_ptr, reinterpret_cast<const int32_t*>(pk->d_pcol), pk->d_diag, X, Z, V, Y, p, \
+      q, r, c, rows_per_cta, vt)
+#define POLFED_GO(UZ, UV)                                                                        \
+  if (nv == 1) POLFED_PK(UZ, UV, 1);                                                             \
+  else if (nv == 2) POLFED_PK(UZ, UV, 2);                                                        \
+  else                                                                                           \
+    fused_step_kernel<S, VEC, UZ, UV, 0><<<grid, kThreads, 0, st>>>(                             \
+        n, ham->d_row_ptr, ham->d_col, ham->d_val, X, Z, V, Y, p, q, r, c, rows_per_cta, vt)
+  if (uz && uv) { POLFED_GO(true, true); }
+  else if (uz) { POLFED_GO(true, false); }
+  else if (uv) { POLFED_GO(false, true); }
+  else { POLFED_GO(false, false); }
 #undef POLFED_GO
+#undef POLFED_PK
   POLFED_LAUNCH_CHECK("fused_step_kernel");
   return POLFED_OK;
 }
