@@ -269,10 +269,10 @@ def run_cuda(args):
     flip = args.format == "flip" or (args.format == "auto" and w.n_up < 0 and w.s in (8, 16, 32)
                                      and all(t[0] in ("XX", "Z", "ZZ") for t in w.terms))
     fmt_name = "tiled" if tiled else ("flip" if flip else
-                                      (args.format if args.format in ("sell", "sector") else "csr"))
+                                      ("sector" if args.format == "sector" else "csr"))
     ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense,
                                      fmt={"tiled": P.FORMAT_TILED, "flip": P.FORMAT_FLIP,
-                                          "sell": P.FORMAT_SELL, "csr": P.FORMAT_CSR,
+                                          "csr": P.FORMAT_CSR,
                                           "sector": P.FORMAT_SECTOR}[fmt_name])
     tiled = tiled or fmt_name == "sector"     # same launch structure and timing method
     torch.cuda.synchronize()
@@ -386,7 +386,7 @@ def run_cuda(args):
             "clocks": clocks.summary(),
             "roofline": {"bound": "hbm",
                          "kernel": {"tiled": "tiled_sweep_kernel", "flip": "flip_step_kernel",
-                                    "sell": "sell_step_kernel", "sector": "sector_sweep_kernel",
+                                    "sector": "sector_sweep_kernel",
                                     "csr": "fused_step_kernel"}[fmt_name], "achieved": achieved,
                          "peak": peak, "peak_source": peak_src, "unit": UNIT,
                          "frac": achieved / peak, "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS,
@@ -520,7 +520,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--per-config", default="1,2,3,4",
                     help="other configs whose fused launch is timed at N=1 ('' to skip)")
-    ap.add_argument("--format", default="auto", choices=["auto", "csr", "sell", "tiled", "flip", "sector"],
+    ap.add_argument("--format", default="auto", choices=["auto", "csr", "tiled", "flip", "sector"],
                     help="auto: tiled where supported and n_sites >= 24, flip for full-space XX models, "
                          "else CSR")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -99,7 +99,7 @@ typedef struct {
 
 enum {
   POLFED_FORMAT_CSR = 0,
-  POLFED_FORMAT_SELL = 1,  /* CSR plus SELL-8-sigma, see below */
+  /* 1 was SELL-8-sigma in round 1: slower than the CSR kernel on every config, removed */
   POLFED_FORMAT_TILED = 2, /* CSR plus the tiled structured format below */
   POLFED_FORMAT_FLIP = 3,  /* CSR plus the matrix-free flip format below */
   POLFED_FORMAT_SECTOR = 4 /* the tiled format with register-resident tile-local hops, below */
@@ -144,16 +144,6 @@ int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_ter
  * beyond POLFED_FORMAT_TILED's (else POLFED_EINVAL): the bond pattern above in both row orders,
  * at most 3 hopping terms across the cut, ceil(n_sites/2) in {4..9, 13} (chains with (i, i+2)
  * bonds) or {6, 7, 8, 10} (without).  Same alignment rules and workspace ownership. */
-
-/* POLFED_FORMAT_SELL (SELL-C-sigma, C = 8, sigma = 128): besides the CSR, the handle keeps the
- * rows sorted by falling length inside windows of 128 rows, cut into slices of 8 rows stored
- * column-major and padded to the longest row of the slice.  Every fused step on the handle with
- * s in {8, 16, 32} (for s >= 16: blocks aligned to 32 bytes, else the CSR kernel runs) reads its
- * entries from these slices: four lanes per row, a warp per slice, entries addressed directly
- * instead of broadcast by shuffles.  Any term list; same result as the CSR kernel (same order of
- * the row sum).  Costs a second copy of the matrix (12 bytes per stored entry plus padding).
- * Measured slower than the CSR kernel on configs 3 and 5: an evaluated
- * alternative, not the default. */
 
 /* POLFED_FORMAT_FLIP (matrix-free rows for full-space spin models, the paper's Fig. 7 kernel
  * `newstate = state XOR mask`; the quantum sun Eq. 67): besides the CSR, the

@@ -4,7 +4,7 @@ many-body Hamiltonian) as hand-written sm_100a kernels behind a C ABI (include/p
 The functions re-exported here are thin ctypes wrappers with the names of the C entry points.
 """
 from .binding import (  # noqa: F401
-    Basis, Ham, PolfedError, EXPORTS, LIB_PATH, TERM_KINDS, FORMAT_CSR, FORMAT_SELL, FORMAT_TILED, FORMAT_FLIP, FORMAT_SECTOR,
+    Basis, Ham, PolfedError, EXPORTS, LIB_PATH, TERM_KINDS, FORMAT_CSR, FORMAT_TILED, FORMAT_FLIP, FORMAT_SECTOR,
     lib, polfed_last_error, polfed_version,
     polfed_build_basis, polfed_basis_dim, polfed_basis_states, polfed_basis_rank,
     polfed_build_hamiltonian, polfed_ham_from_csr, polfed_ham_csr,

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libpolfed.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ERANGE, ENOCONV, EBREAKDOWN = range(7)
 TERM_KINDS = {"ZZ": 0, "Z": 1, "NN": 2, "N": 3, "EXCH": 4, "HOPJW": 5, "XX": 6}
-FORMAT_CSR, FORMAT_SELL, FORMAT_TILED, FORMAT_FLIP, FORMAT_SECTOR = 0, 1, 2, 3, 4
+FORMAT_CSR, FORMAT_TILED, FORMAT_FLIP, FORMAT_SECTOR = 0, 2, 3, 4
 
 EXPORTS = (
     "polfed_last_error", "polfed_version",

@@ -83,7 +83,6 @@ int polfed_ham_destroy(polfed_ham* ham) {
   if (!ham) return POLFED_OK;
   polfed::destroy_tiled_plan(ham->tiled);
   polfed::destroy_flip_plan(ham->flip);
-  polfed::destroy_sell_plan(ham->sell);
   polfed::destroy_packed_plan(ham->packed);
   if (ham->owns) {
     cudaFree(const_cast<int32_t*>(ham->d_row_ptr));

@@ -269,8 +269,8 @@ extern "C" int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_
   if (!out) return fail(POLFED_EINVAL, "polfed_build_hamiltonian: out is NULL");
   *out = nullptr;
   if (!basis) return fail(POLFED_EINVAL, "polfed_build_hamiltonian: basis is NULL");
-  if (format < POLFED_FORMAT_CSR || format > POLFED_FORMAT_SECTOR)
-    return fail(POLFED_EINVAL, "polfed_build_hamiltonian: format must be POLFED_FORMAT_CSR, _SELL, "
+  if (format != POLFED_FORMAT_CSR && (format < POLFED_FORMAT_TILED || format > POLFED_FORMAT_SECTOR))
+    return fail(POLFED_EINVAL, "polfed_build_hamiltonian: format must be POLFED_FORMAT_CSR, "
                                "_TILED, _FLIP or _SECTOR");
   if (n_terms < 0 || (n_terms > 0 && !h_terms))
     return fail(POLFED_EINVAL, "polfed_build_hamiltonian: bad term list");
@@ -319,13 +319,6 @@ extern "C" int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_
   h->owns = true;
   if (format == POLFED_FORMAT_TILED || format == POLFED_FORMAT_SECTOR) {
     rc = build_tiled_plan(basis, terms, format == POLFED_FORMAT_SECTOR, st, &h->tiled);
-    if (rc) {
-      polfed_ham_destroy(h);
-      return rc;
-    }
-  }
-  if (format == POLFED_FORMAT_SELL) {
-    rc = build_sell_plan(h, st, &h->sell);
     if (rc) {
       polfed_ham_destroy(h);
       return rc;

@@ -51,7 +51,6 @@ struct DevTerm {
 
 struct TiledPlan;  // tiled.cuh
 struct FlipPlan;   // flip.cuh
-struct SellPlan;   // sell.cuh
 struct PackedPlan; // packed.cuh
 
 // assemble.cu: CSR of a term list over a basis; arrays cudaMalloc'ed, owned by the caller.
@@ -75,14 +74,6 @@ bool flip_supports(const polfed_ham* ham, int s);
 int flip_step(const polfed_ham* ham, int s, double p, double q, double r, double c, const double* X,
               const double* Z, const double* V, double* Y, cudaStream_t st);
 
-// sell.cu: SELL-8-sigma, see sell.cuh.
-int build_sell_plan(const polfed_ham* ham, cudaStream_t st, SellPlan** out);
-void destroy_sell_plan(SellPlan* plan);
-bool sell_supports(const polfed_ham* ham, int s, const void* X, const void* Z, const void* V,
-                   const void* Y);
-int sell_step(const polfed_ham* ham, int s, double p, double q, double r, double c, const double* X,
-              const double* Z, const double* V, double* Y, cudaStream_t st);
-
 // small_filter.cu: the whole recurrence in one persistent single-CTA kernel (n * s <= 4096).
 // small_filter_apply returns POLFED_ERANGE when the rows do not fit its shared memory.
 bool small_filter_supports(const polfed_ham* ham, int s);
@@ -91,8 +82,7 @@ int small_filter_apply(const polfed_ham* ham, double a, double b, int K, const d
                        int s, const double* d_V, double* d_W, double* cur, double* old,
                        cudaStream_t st);
 
-// spmm_clenshaw.cu: the fused step without argument validation (flip handles: flip_step, SELL
-// handles: sell_step).
+// spmm_clenshaw.cu: the fused step without argument validation (flip handles: flip_step).
 int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
                   const double* X, const double* Z, const double* V, double* Y, cudaStream_t st);
 
@@ -129,6 +119,5 @@ struct polfed_ham {
   int max_row_len = 0;   // longest CSR row (small_filter.cu)
   polfed::TiledPlan* tiled = nullptr;  // POLFED_FORMAT_TILED only (owned)
   polfed::FlipPlan* flip = nullptr;    // POLFED_FORMAT_FLIP only (owned)
-  polfed::SellPlan* sell = nullptr;    // POLFED_FORMAT_SELL only (owned)
   polfed::PackedPlan* packed = nullptr;  // every handle whose matrix qualifies (owned)
 };

@@ -151,7 +151,7 @@ const void* const kKernels[4] = {
 
 // True when the persistent kernel takes the recurrence of this handle and block size.
 bool small_filter_supports(const polfed_ham* ham, int s) {
-  if (!ham || ham->tiled || ham->flip || ham->sell || ham->max_row_len < 1) return false;
+  if (!ham || ham->tiled || ham->flip || ham->max_row_len < 1) return false;
   return ham->n * (long long)s <= kSingleItems;
 }
 

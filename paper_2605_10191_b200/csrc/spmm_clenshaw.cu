@@ -263,8 +263,6 @@ int launch_step(const polfed_ham* ham, double p, double q, double r, double c, c
 int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
                   const double* X, const double* Z, const double* V, double* Y, cudaStream_t st) {
   if (flip_supports(ham, s)) return flip_step(ham, s, p, q, r, c, X, Z, V, Y, st);
-  if (sell_supports(ham, s, X, r != 0.0 ? Z : nullptr, c != 0.0 ? V : nullptr, Y))
-    return sell_step(ham, s, p, q, r, c, X, Z, V, Y, st);
   switch (s) {
     case 1: return launch_step<1>(ham, p, q, r, c, X, Z, V, Y, st);
     case 2: return launch_step<2>(ham, p, q, r, c, X, Z, V, Y, st);
