@@ -310,7 +310,7 @@ __device__ __forceinline__ void structured_v1(const SecArgs& a, int k, const uin
   const double at1 = alpha * a.t1, at2 = alpha * a.t2;
   const int nu1 = a.tab.n_units[0][k];
   for (int u = claim(ctr, 1, lane); u < nu1; u = claim(ctr, 1, lane)) {
-    const int unit = __ldg(units1 + u), j1 = unit & 7, i2 = (unit >> 3) * kSecGroups + grp;
+    const int unit = units1[u], j1 = unit & 7, i2 = (unit >> 3) * kSecGroups + grp;
     if (i2 < a.tab.n2[k - j1]) {
       const uint32_t off = (uint32_t)(a.tab.srow[k][j1] + i2 * a.tab.n1p[j1]) * 64u;
       view1_dispatch<G1, NNN, JW>(j1, src + off, dst + off, at1, at2, beta, gamma, use_old, epoch,
@@ -328,7 +328,7 @@ __device__ __forceinline__ void structured_v2(const SecArgs& a, int k, const uin
   const double at1 = alpha * a.t1, at2 = alpha * a.t2;
   const int nu2 = a.tab.n_units[1][k];
   for (int u = claim(ctr, 1, lane); u < nu2; u = claim(ctr, 1, lane)) {
-    const int unit = __ldg(units2 + u), j1 = unit & 7, i1 = (unit >> 3) * kSecGroups + grp;
+    const int unit = units2[u], j1 = unit & 7, i1 = (unit >> 3) * kSecGroups + grp;
     if (i1 < a.tab.n1[j1]) {
       const uint32_t off = (uint32_t)(a.tab.srow[k][j1] + i1) * 64u;
       view2_dispatch<G2, NNN, JW>(k - j1, src + off, dst + off, (uint32_t)a.tab.n1p[j1] * 64u, at1,
@@ -398,8 +398,7 @@ __device__ __forceinline__ void l2_prefetch(const void* p, unsigned bytes, int t
 
 constexpr int kTailRows = 8;  // rows per warp iteration of the row passes: 4 lanes x 16 bytes each
 constexpr int kSecWarps = kSecThreads / 32;
-// Row passes: register sets, look-ahead of the row records and of the cross-cut operands.
-constexpr int kD = 6, kDM = 5, kDO = 2;
+constexpr int kBatch = 3;  // row passes: 8-row groups per warp and batch
 
 template <int M, bool NNN, bool JW, int MODE>
 __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecArgs a) {
@@ -407,7 +406,8 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ uint64_t bar;
   __shared__ int4 s_work[2];  // work item, first row, rows, class of the tile
-  __shared__ int s_ctr[4];
+  __shared__ uint16_t s_units[2 * (M + 1) * kSecMaxUnits];
+  __shared__ int s_ctr[6];  // per tile: view 1, view 2, row pass of phase 2; the same of phase 3
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int l8 = lane & 7;                   // structured passes: 8 lanes x 8 bytes per row
   const int q = lane & 3, slot = lane >> 2;  // row passes: 4 lanes x 16 bytes per row
@@ -422,6 +422,7 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
     }
     return w;
   };
+  for (int i = tid; i < 2 * (M + 1) * kSecMaxUnits; i += kSecThreads) s_units[i] = a.units[i];
   if (tid == 0) {
     mbar_init(&bar, 1);
     s_work[0] = next_work();
@@ -439,7 +440,7 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
     const int work = wi.x, row0 = wi.y, nrows = wi.z, k = wi.w;
     if (work >= total) break;
     const int panel = work / a.n_tiles;
-    if (tid == 0) s_ctr[0] = s_ctr[1] = s_ctr[2] = s_ctr[3] = 0;
+    if (tid < 6) s_ctr[tid] = 0;
     if (MODE != MODE_INIT && warp == 0) {
       // the tile panels of b_{k+1} -> buffer A and of the partial b_k -> buffer B: one bulk copy
       // each, or one per fibre when the fibre pitch is padded
@@ -451,7 +452,7 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
       const size_t off = panel * panel_stride + (size_t)row0 * kSecPanel;
       if (a.tab.rows_p[k] == nrows) {  // no padding: the whole tile is one run
         if (lane < 2)
-          bulk_g2s(lane ? sB : sA, (lane ? a.Pk : a.X1) + off, (unsigned)nrows * 64u, &bar, pol_last);
+          bulk_g2s(lane ? sB : sA, (lane ? a.Pk : a.X1) + off, (unsigned)nrows * 64u, &bar, lane ? pol_first : pol_last);
       } else {
         const int j_lo = k > G2 ? k - G2 : 0, j_hi = k < G1 ? k : G1;
         for (int j1 = j_lo; j1 <= j_hi; ++j1) {
@@ -461,7 +462,7 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
             const int i2 = i >> 1;
             const double* src = ((i & 1) ? a.Pk : a.X1) + off + (size_t)(p0 + i2 * n1) * kSecPanel;
             bulk_g2s(((i & 1) ? sB : sA) + (unsigned)(r0 + i2 * n1p) * 64u, src, (unsigned)n1 * 64u,
-                     &bar, pol_last);
+                     &bar, (i & 1) ? pol_first : pol_last);
           }
         }
       }
@@ -471,9 +472,9 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
     const double* V = a.V + panel * panel_stride + (size_t)row0 * kSecPanel + 2 * q;
     double* Bout = a.Bout + panel * panel_stride + 2 * q;
     double* Pout = a.Pout + panel * panel_stride + 2 * q;
-    const uint16_t* units1 = a.units + (size_t)k * kSecMaxUnits;
-    const uint16_t* units2 = a.units + (size_t)(M + 1 + k) * kSecMaxUnits;
-    // the rows of the row passes are dealt out statically: chunk c of 8 rows -> warp c mod warps
+    const uint16_t* units1 = s_units + k * kSecMaxUnits;
+    const uint16_t* units2 = s_units + (M + 1 + k) * kSecMaxUnits;
+    // MODE_INIT: rows dealt out statically, 8 per warp and turn
     const int pos0 = warp * kTailRows + slot;
     constexpr int kStride = kSecWarps * kTailRows;
     __syncthreads();  // counters reset
@@ -513,44 +514,44 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
           if (a.cs != 0.0) l2_prefetch(a.V + off, bytes, tid, (per + 1) / 2);
         }
       }
-      // Row passes are software-pipelined over three register sets (static indices: the loop
-      // body is unrolled three times): row records two iterations ahead, the global operands of
-      // a row (P_k or V, cross-cut partners) one iteration ahead; the first of them are
-      // requested before the structured passes, which hide their latency.
-      RowMeta m[kD];
-      m[0] = load_meta(meta, pos0, nrows, p2);
-      m[1] = load_meta(meta, pos0 + kStride, nrows, p2);
+      // Row passes work in batches of kBatch x 8 rows per warp (rows dealt out statically: batch t
+      // of warp w starts at row (t * warps + w) * 32): all row records of a batch are requested
+      // at once, then all global operands, then the rows are finished.  Few load generations
+      // with many loads each suit the six scoreboards of a warp; the records of the warp's rows
+      // are asked into L1 before the structured passes, which hide that latency.
+      constexpr int kBatchRows = kBatch * kTailRows;
       if (p2) {
         mbar_wait(&bar, parity);
         parity ^= 1u;
       }
-      structured_v1<G1, NNN, JW>(a, k, units1, &s_ctr[p2 ? 0 : 2], (p2 ? sA : sB) + 8u * l8,
+      structured_v1<G1, NNN, JW>(a, k, units1, &s_ctr[p2 ? 0 : 3], (p2 ? sA : sB) + 8u * l8,
                                  (p2 ? sB : sA) + 8u * l8, p2 ? a.pf : a.ps, p2 ? 0.0 : a.qs,
                                  p2 ? 1.0 : a.rs, p2 || MODE != MODE_INIT, epoch, lane);
+      structured_v2<G2, NNN, JW>(a, k, units2, &s_ctr[p2 ? 1 : 4], (p2 ? sA : sB) + 8u * l8,
+                                 (p2 ? sB : sA) + 8u * l8, p2 ? a.pf : a.ps, epoch, lane);
+      // two register sets in turn (A, B): the records of the next batch are requested before the
+      // rows of the current one are finished
       if (p2) {
-        RowOperands o[kD];
-        o[0] = load_operands(m[0], X1);
-        structured_v2<G2, NNN, JW>(a, k, units2, &s_ctr[1], sA + 8u * l8, sB + 8u * l8, a.pf, epoch,
-                                   lane);
+        auto load_m = [&](RowMeta (&m)[kBatch], int base) {
 #pragma unroll
-        for (int j = 2; j < kDM; ++j) m[j] = load_meta(meta, pos0 + j * kStride, nrows, true);
+          for (int u = 0; u < kBatch; ++u) m[u] = load_meta(meta, base + slot + u * kTailRows, nrows, true);
+        };
+        auto load_o = [&](RowOperands (&o)[kBatch], const RowMeta (&m)[kBatch]) {
 #pragma unroll
-        for (int j = 1; j < kDO; ++j) o[j] = load_operands(m[j], X1);
-        for (int base = warp * kTailRows; base < nrows;) {  // warp-uniform loop control
+          for (int u = 0; u < kBatch; ++u) o[u] = load_operands(m[u], X1);
+        };
+        auto finish = [&](int base, const RowMeta (&m)[kBatch], const RowOperands (&o)[kBatch]) {
 #pragma unroll
-          for (int j = 0; j < kD; ++j) {
-            const int pos = base + slot;
-            if (base >= nrows) break;
-            m[(j + kDM) % kD] = load_meta(meta, pos + kDM * kStride, nrows, true);
-            o[(j + kDO) % kD] = load_operands(m[(j + kDO) % kD], X1);
-            const uint32_t c0 = m[j].m0.w, c1 = m[j].m1.x, c2 = m[j].m1.y;
-            const uint32_t own = (m[j].m0.z >> 16) * 64u + 16u * q;
+          for (int u = 0; u < kBatch; ++u) {
+            const int pos = base + slot + u * kTailRows;
+            const uint32_t c0 = m[u].m0.w, c1 = m[u].m1.x, c2 = m[u].m1.y;
+            const uint32_t own = (m[u].m0.z >> 16) * 64u + 16u * q;
             double2 y = make_double2(0.0, 0.0);
-            fma2(__hiloint2double((int)m[j].m1.w, (int)m[j].m1.z), lds128(sA + own, epoch), y);
-            cross_group(m[j], sA + 16u * q, a.t1, a.t2, epoch, y);
-            fma2(signed_coef(a.ccoef[(c0 >> kCrossPosBits) & 15u], c0), o[j].h0, y);
-            fma2(signed_coef(a.ccoef[(c1 >> kCrossPosBits) & 15u], c1), o[j].h1, y);
-            fma2(signed_coef(a.ccoef[(c2 >> kCrossPosBits) & 15u], c2), o[j].h2, y);
+            fma2(__hiloint2double((int)m[u].m1.w, (int)m[u].m1.z), lds128(sA + own, epoch), y);
+            cross_group(m[u], sA + 16u * q, a.t1, a.t2, epoch, y);
+            fma2(signed_coef(a.ccoef[(c0 >> kCrossPosBits) & 15u], c0), o[u].h0, y);
+            fma2(signed_coef(a.ccoef[(c1 >> kCrossPosBits) & 15u], c1), o[u].h1, y);
+            fma2(signed_coef(a.ccoef[(c2 >> kCrossPosBits) & 15u], c2), o[u].h2, y);
             double2 b = lds128(sB + own, epoch);  // P_k + pf O_l b_{k+1}
             b.x = fma(a.pf, y.x, b.x);
             b.y = fma(a.pf, y.y, b.y);
@@ -559,40 +560,62 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
                 const int dst = __ldg(a.dst_nat + row0 + pos);
                 stg128_stream(a.W + (size_t)dst * a.w_ld + panel * kSecPanel + 2 * q, b, pol_first);
               } else {
-                stg128_stream(Bout + (size_t)m[j].m0.x * kSecPanel, b, pol_first);
+                stg128_stream(Bout + (size_t)m[u].m0.x * kSecPanel, b, pol_first);
                 sts128(sB + own, b);
               }
             }
-            base += kStride;
           }
+        };
+        RowMeta mA[kBatch], mB[kBatch];
+        RowOperands oA[kBatch], oB[kBatch];
+        int baseA = claim(&s_ctr[2], kBatchRows, lane), baseB;
+        load_m(mA, baseA);
+        for (;;) {
+          if (baseA >= nrows) break;
+          baseB = claim(&s_ctr[2], kBatchRows, lane);
+          load_o(oA, mA);
+          load_m(mB, baseB);
+          finish(baseA, mA, oA);
+          if (baseB >= nrows) break;
+          baseA = claim(&s_ctr[2], kBatchRows, lane);
+          load_o(oB, mB);
+          load_m(mA, baseA);
+          finish(baseB, mB, oB);
         }
       } else {
         const bool use_v = a.cs != 0.0;
-        double2 v[kD];
-        v[0] = load_stream_if(V, pos0, nrows, use_v, pol_first);
-        v[1] = load_stream_if(V, pos0 + kStride, nrows, use_v, pol_first);
-        structured_v2<G2, NNN, JW>(a, k, units2, &s_ctr[3], sB + 8u * l8, sA + 8u * l8, a.ps, epoch,
-                                   lane);
+        auto load_mv = [&](RowMeta (&m)[kBatch], double2 (&v)[kBatch], int base) {
 #pragma unroll
-        for (int j = 2; j < kDM; ++j) {
-          m[j] = load_meta(meta, pos0 + j * kStride, nrows, false);
-          v[j] = load_stream_if(V, pos0 + j * kStride, nrows, use_v, pol_first);
-        }
-        for (int base = warp * kTailRows; base < nrows;) {  // warp-uniform loop control
-#pragma unroll
-          for (int j = 0; j < kD; ++j) {
-            const int pos = base + slot;
-            if (base >= nrows) break;
-            m[(j + kDM) % kD] = load_meta(meta, pos + kDM * kStride, nrows, false);
-            v[(j + kDM) % kD] = load_stream_if(V, pos + kDM * kStride, nrows, use_v, pol_first);
-            const uint32_t own = (m[j].m0.z >> 16) * 64u + 16u * q;
-            double2 z = lds128(sA + own, epoch), g = make_double2(0.0, 0.0);
-            cross_group(m[j], sB + 16u * q, a.t1, a.t2, epoch, g);
-            z.x = fma(a.cs, v[j].x, fma(a.ps, g.x, z.x));
-            z.y = fma(a.cs, v[j].y, fma(a.ps, g.y, z.y));
-            if (pos < nrows) stg128_stream(Pout + (size_t)m[j].m0.x * kSecPanel, z, pol_first);
-            base += kStride;
+          for (int u = 0; u < kBatch; ++u) {
+            m[u] = load_meta(meta, base + slot + u * kTailRows, nrows, false);
+            v[u] = load_stream_if(V, base + slot + u * kTailRows, nrows, use_v, pol_first);
           }
+        };
+        auto finish = [&](int base, const RowMeta (&m)[kBatch], const double2 (&v)[kBatch]) {
+#pragma unroll
+          for (int u = 0; u < kBatch; ++u) {
+            const int pos = base + slot + u * kTailRows;
+            const uint32_t own = (m[u].m0.z >> 16) * 64u + 16u * q;
+            double2 z = lds128(sA + own, epoch), g = make_double2(0.0, 0.0);
+            cross_group(m[u], sB + 16u * q, a.t1, a.t2, epoch, g);
+            z.x = fma(a.cs, v[u].x, fma(a.ps, g.x, z.x));
+            z.y = fma(a.cs, v[u].y, fma(a.ps, g.y, z.y));
+            if (pos < nrows) stg128_stream(Pout + (size_t)m[u].m0.x * kSecPanel, z, pol_first);
+          }
+        };
+        RowMeta mA[kBatch], mB[kBatch];
+        double2 vA[kBatch], vB[kBatch];
+        int baseA = claim(&s_ctr[5], kBatchRows, lane), baseB;
+        load_mv(mA, vA, baseA);
+        for (;;) {
+          if (baseA >= nrows) break;
+          baseB = claim(&s_ctr[5], kBatchRows, lane);
+          load_mv(mB, vB, baseB);
+          finish(baseA, mA, vA);
+          if (baseB >= nrows) break;
+          baseA = claim(&s_ctr[5], kBatchRows, lane);
+          load_mv(mA, vA, baseA);
+          finish(baseB, mB, vB);
         }
       }
       __syncthreads();  // after phase 3: both buffers are free for the next tile
