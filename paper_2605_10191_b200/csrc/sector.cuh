@@ -24,6 +24,10 @@ constexpr int kSecPanel = 8;       // columns per panel: 64-byte rows
 constexpr int kSecMaxG = 7;        // sites per group (C(7,3) = 35 rows of a fibre in registers)
 constexpr int kSecThreads = 512;
 constexpr int kSecMaxUnits = 48;   // work units per class and view
+// Sites of the low group G1.  C(g1, j) should be odd for every j (g1 = 2^t - 1): four G1-fibres
+// that a warp reads together then start at alternating 64-byte halves of the 128-byte bank row,
+// so view 1 is free of bank conflicts without any padding.  m = 13 -> 7 + 6, m = 7 -> 3 + 4.
+constexpr int sector_g1(int m) { return m >= 10 ? 7 : (m >= 4 ? 3 : 1); }
 constexpr int kSecGroups = 4;      // lane groups (fibres) per warp: 8 lanes x 8 bytes per row
 
 // cross-group entry (16 bits; slot 0: the (g1-1, g1) bond with amplitude t1, slots 1 and 2: the

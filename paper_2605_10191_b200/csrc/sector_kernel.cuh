@@ -402,12 +402,14 @@ constexpr int kBatch = 3;  // row passes: 8-row groups per warp and batch
 
 template <int M, bool NNN, bool JW, int MODE>
 __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecArgs a) {
-  constexpr int G1 = M / 2, G2 = M - G1;
+  constexpr int G1 = sector_g1(M), G2 = M - G1;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ uint64_t bar;
   __shared__ int4 s_work[2];  // work item, first row, rows, class of the tile
   __shared__ uint16_t s_units[2 * (M + 1) * kSecMaxUnits];
-  __shared__ int s_ctr[6];  // per tile: view 1, view 2, row pass of phase 2; the same of phase 3
+  // work counters per tile (view 1, view 2, row pass of phase 2; the same of phase 3), one set per
+  // tile parity: a tile zeroes the other set, so no barrier is needed at the top of a tile
+  __shared__ int s_ctr_all[2][6];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int l8 = lane & 7;                   // structured passes: 8 lanes x 8 bytes per row
   const int q = lane & 3, slot = lane >> 2;  // row passes: 4 lanes x 16 bytes per row
@@ -415,7 +417,7 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
   auto next_work = [&]() {  // one thread: claim a work item and look its tile up
     int4 w = make_int4(atomicAdd(a.counter, 1), 0, 0, 0);
     if (w.x < total) {
-      const int tile = w.x % a.n_tiles;
+      const int tile = w.x / a.n_panels;
       w.y = __ldg(a.tile_row0 + tile);
       w.z = __ldg(a.tile_row0 + tile + 1) - w.y;
       w.w = __ldg(a.tile_class + tile);
@@ -423,6 +425,7 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
     return w;
   };
   for (int i = tid; i < 2 * (M + 1) * kSecMaxUnits; i += kSecThreads) s_units[i] = a.units[i];
+  if (tid < 12) s_ctr_all[tid / 6][tid % 6] = 0;
   if (tid == 0) {
     mbar_init(&bar, 1);
     s_work[0] = next_work();
@@ -435,12 +438,14 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
   const uint32_t sA = smem_u32(smem_raw), sB = sA + a.buf_bytes;
 
   for (int it = 0;; ++it) {
-    // work items in panel-major order: all tiles of panel 0, then panel 1, ...
+    // work items in tile-major order: the s/8 panels of a tile are consecutive items, so they run at
+    // about the same time on different SMs and share the tile's row records in L2
     const int4 wi = s_work[it & 1];
     const int work = wi.x, row0 = wi.y, nrows = wi.z, k = wi.w;
     if (work >= total) break;
-    const int panel = work / a.n_tiles;
-    if (tid < 6) s_ctr[tid] = 0;
+    const int panel = work % a.n_panels;
+    int* const s_ctr = s_ctr_all[it & 1];
+    if (tid < 6) s_ctr_all[(it + 1) & 1][tid] = 0;
     if (MODE != MODE_INIT && warp == 0) {
       // the tile panels of b_{k+1} -> buffer A and of the partial b_k -> buffer B: one bulk copy
       // each, or one per fibre when the fibre pitch is padded
@@ -477,8 +482,6 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
     // MODE_INIT: rows dealt out statically, 8 per warp and turn
     const int pos0 = warp * kTailRows + slot;
     constexpr int kStride = kSecWarps * kTailRows;
-    __syncthreads();  // counters reset
-    ++epoch;
     // The next work item is claimed by the last warp (only its lane 0 waits for the atomic) and
     // read after later barriers.
     if (tid == kSecThreads - 32) s_work[(it + 1) & 1] = next_work();
@@ -506,7 +509,7 @@ __global__ void __launch_bounds__(kSecThreads, 1) sector_sweep_kernel(const SecA
       if (!p2) {  // row records and V of the next work item -> L2
         const int4 wn = s_work[(it + 1) & 1];
         if (wn.x < total) {
-          const int panel_n = wn.x / a.n_tiles, r0n = wn.y;
+          const int panel_n = wn.x % a.n_panels, r0n = wn.y;
           const unsigned bytes = (unsigned)wn.z * 64u;
           const size_t off = panel_n * panel_stride + (size_t)r0n * kSecPanel;
           const int per = (int)((bytes + 2047u) / 2048u);

@@ -277,7 +277,7 @@ struct SectorHost {
 
 // Geometry shared by both layouts: sector bases, fibre pitches, work units.
 void sector_geometry(int m, bool pad, SectorPlan* sp, std::vector<uint16_t>* units) {
-  const int g1 = m / 2, g2 = m - g1;
+  const int g1 = sector_g1(m), g2 = m - g1;
   sp->m = m;
   sp->g1 = g1;
   sp->g2 = g2;
