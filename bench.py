@@ -402,6 +402,9 @@ def run_cuda(args):
             if args.config == 5 and fmt_name == "tiled":   # the evaluated alternative (DESIGN 5d)
                 line["per_config"].append(hot_path_on_config(P, 5, peak, "sector"))
             torch.cuda.empty_cache()
+        if world == 1 and not args.no_reorth:
+            line["reorth"] = reorth_timing(P, n, s, peak)
+            torch.cuda.empty_cache()
         if world == 1 and args.eigs:
             torch.cuda.empty_cache()
             line["seconds_to_nev"] = [time_to_nev(P, int(c)) for c in args.eigs.split(",") if c]
@@ -480,6 +483,41 @@ def hot_path_on_config(P, config: int, peak: float, fmt_name: str = ""):
             "l2": "inputs exceed L2" if by > 4 * 126e6 else "working set fits L2 (not flushed)"}
 
 
+def reorth_timing(P, n: int, s: int, peak: float, k: int = 8):
+    """The two tall-skinny products of the full reorthogonalisation (Eq. 9, 11 PAPER.md:147-153) at
+    this workload's size against k basis panels: C_j = Q_j^T W and W -= sum_j Q_j C_j, CUDA events,
+    best of 5.  Bytes: Q once plus W (read; the update also writes it)."""
+    import torch
+    Q = torch.randn(k, n, s, dtype=torch.float64, device="cuda")
+    B = torch.randn(n, s, dtype=torch.float64, device="cuda")
+
+    def timed(f):
+        f()
+        torch.cuda.synchronize()
+        best = float("inf")
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            f()
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        return best
+
+    out = {"n": n, "s": s, "panels": k}
+    for name, variant in (("gram_fma", 1), ("gram_tensor", 2)):
+        ms = timed(lambda: P.polfed_block_gram(Q, B, variant=variant))
+        by = 8 * n * s * (k + 1)
+        out[name] = {"ms": ms, "gbs": by / ms / 1e6, "frac_of_measured": by / ms / 1e6 / peak,
+                     "fp64_tflops": 2.0 * n * s * s * k / ms / 1e9}
+    C = P.polfed_block_gram(Q, B)
+    ms = timed(lambda: P.polfed_block_update(Q, C, B, -1.0, 1.0))
+    by = 8 * n * s * (k + 2)
+    out["update_tensor"] = {"ms": ms, "gbs": by / ms / 1e6, "frac_of_measured": by / ms / 1e6 / peak,
+                            "fp64_tflops": 2.0 * n * s * s * k / ms / 1e9}
+    return out
+
+
 def time_to_nev(P, config: int):
     """Second half of BASELINE.json's metric: wall seconds of polfed_block_lanczos_eigs (bounds,
     order rule, block Lanczos on P(H~), Rayleigh-Ritz, residuals) for the workload's nev pairs."""
@@ -524,6 +562,8 @@ def main():
                     help="auto: tiled where supported and n_sites >= 24, flip for full-space XX models, "
                          "else CSR")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-reorth", action="store_true",
+                    help="skip the timing of the reorthogonalisation products")
     ap.add_argument("--eigs", default="1,2,3",
                     help="configs whose full eigen-solve is timed at N=1 ('' to skip; 4 takes minutes)")
     args = ap.parse_args()

@@ -312,16 +312,27 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
   constexpr int kIterRows = (THREADS / 32) * kRowsPerIter;  // rows per CTA pass (static loops)
   extern __shared__ __align__(128) unsigned char smem_raw[];  // (max_tile_rows + 1) x 128 B
   __shared__ uint64_t bar;
-  __shared__ int s_tile[2];
+  __shared__ int4 s_tile[2];  // work item, first row, rows, first record of the tile's class
   __shared__ int s_chunk[2];  // next unclaimed position of the running phase / the one after it
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int q = lane & 3, slot = lane >> 2;
   const bool odd = slot & 1;
   const unsigned char* x_first = smem_raw + 32 * q + (odd ? 16 : 0);
   const unsigned char* x_second = smem_raw + 32 * q + (odd ? 0 : 16);
+  const int total = a.n_tiles * a.n_panels;
+  auto next_work = [&]() {  // one thread: claim a work item and look its tile up
+    int4 w = make_int4(atomicAdd(a.counter, 1), 0, 0, 0);
+    if (w.x < total) {
+      const int tile = w.x % a.n_tiles;
+      w.y = __ldg(a.tile_row0 + tile);
+      w.z = __ldg(a.tile_row0 + tile + 1) - w.y;
+      w.w = __ldg(a.tile_rec0 + tile);
+    }
+    return w;
+  };
   if (tid == 0) {
     mbar_init(&bar, 1);
-    s_tile[0] = atomicAdd(a.counter, 1);
+    s_tile[0] = next_work();
     s_chunk[0] = s_chunk[1] = 0;
   }
   __syncthreads();
@@ -335,19 +346,19 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
 
   for (int it = 0;; ++it) {
     // work items in panel-major order: all tiles of panel 0, then panel 1 (half the live X in L2)
-    const int work = s_tile[it & 1];
-    if (work >= a.n_tiles * a.n_panels) break;
-    const int tile = work % a.n_tiles, panel_of_work = work / a.n_tiles;
-    if (tid == 0) s_tile[(it + 1) & 1] = atomicAdd(a.counter, 1);  // read after later barriers
-    const int row0 = __ldg(a.tile_row0 + tile);
-    const int nrows = __ldg(a.tile_row0 + tile + 1) - row0;
-    const uint4* rec = reinterpret_cast<const uint4*>(a.records) +
-                       (size_t)__ldg(a.tile_rec0 + tile) * 4;
+    const int4 wi = s_tile[it & 1];
+    const int work = wi.x, row0 = wi.y, nrows = wi.z;
+    if (work >= total) break;
+    const int panel_of_work = work / a.n_tiles;
+    const uint4* rec = reinterpret_cast<const uint4*>(a.records) + (size_t)wi.w * 4;
     const uint32_t* side = a.side + (size_t)row0 * a.side_words;
     const double* diag = a.diag + row0;
     const int32_t* dst_map = a.dst_map + row0;
     if (tid < 8) reinterpret_cast<double2*>(smem_raw)[nrows * 8 + tid] = zero2;  // the zero row
     __syncthreads();
+    // the next work item is claimed by the last warp (only its lane 0 waits for the atomic and the
+    // tile look-up) and read after later barriers
+    if (tid == THREADS - 32) s_tile[(it + 1) & 1] = next_work();
 
     for (int panel = panel_of_work; panel == panel_of_work; ++panel) {
       const double* X1 = a.X1 + panel * panel_stride;
@@ -462,7 +473,7 @@ __global__ void __maxnreg__(THREADS == kTileThreads ? 152 : 80)
       uint4 rq_n = make_uint4(0u, 0u, 0u, 0u);
       if (base + slot < nrows) rq_n = __ldg(rec + (size_t)(base + slot) * 4 + q);
       if (MODE == MODE_STEP)
-        next_work_prefetch(a, s_tile[(it + 1) & 1], panel_stride, tid);
+        next_work_prefetch(a, s_tile[(it + 1) & 1].x, panel_stride, tid);
       mbar_wait(&bar, parity);
       parity ^= 1u;
       // the parked copy is dead once it is back in shared memory: drop it from L2 unwritten
