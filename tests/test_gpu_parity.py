@@ -142,6 +142,60 @@ def test_fused_step_matches_oracle_on_ragged_matrices(P, s, n, avg, empty_every)
         assert np.all(np.abs(got - want) <= 1e-13 * scale)
 
 
+@pytest.mark.parametrize("s", BLOCK_SIZES)
+@pytest.mark.parametrize("values", [(0.5,), (0.5, -1.25), (0.0, 2.0), (0.5, -1.25, 3.0)])
+def test_fused_step_on_matrices_with_few_off_diagonal_values(P, s, values):
+    """The packed form of the CSR (column | value class, dense diagonal: csrc/packed.cu) serves
+    matrices with one or two distinct off-diagonal values; explicit zeros, rows without a stored
+    diagonal, empty rows and a third value (plain CSR again) must all give the same step."""
+    n = 1531
+    rng = np.random.default_rng(len(values) * 100 + s)
+    rows, cols, vals = [], [], []
+    for i in range(n):
+        if i % 11 == 3:
+            continue                                           # an empty row
+        k = int(rng.integers(0, 9))
+        cj = np.unique(rng.integers(0, n, k))
+        cj = cj[cj != i]
+        if i % 5 != 0:                                         # some rows have no stored diagonal
+            rows.append(i); cols.append(i); vals.append(float(rng.standard_normal()))
+        for c in cj:
+            rows.append(i); cols.append(int(c)); vals.append(values[int(rng.integers(0, len(values)))])
+    order = np.lexsort((cols, rows))
+    rows, cols, vals = np.array(rows)[order], np.array(cols, np.int32)[order], np.array(vals)[order]
+    row_ptr = np.zeros(n + 1, np.int32)
+    np.add.at(row_ptr, rows + 1, 1)
+    row_ptr = np.cumsum(row_ptr).astype(np.int32)
+    H = core.CSR(n, row_ptr, cols, vals)
+    X, Z, V = (rng.standard_normal((n, s)) for _ in range(3))
+    ham = ham_from_oracle(P, H)
+    want = 0.7 * core.spmm(H, X) - 0.3 * X - Z + 0.45 * V
+    mag = 0.7 * core.spmm(core.CSR(n, row_ptr, cols, np.abs(vals)), np.abs(X)) + np.abs(X) + np.abs(Z) + np.abs(V)
+    Y = torch.full((n, s), float("nan"), dtype=torch.float64, device="cuda")
+    P.polfed_fused_step(ham, s, 0.7, -0.3, -1.0, 0.45, dev(X), dev(Z), dev(V), Y)
+    assert np.all(np.abs(Y.cpu().numpy() - want) <= 1e-13 * (mag + 1e-300))
+
+
+@pytest.mark.parametrize("n,s,K", [(924, 1, 1000), (1, 1, 5), (300, 8, 385), (513, 4, 384), (4096, 1, 769),
+                                   (128, 32, 50), (4097, 1, 40)])
+def test_filter_on_tiny_matrices_persistent_kernel(P, n, s, K):
+    """n * s <= 4096 runs all K steps inside one persistent kernel per 384 steps
+    (csrc/small_filter.cu); orders that straddle the chunk size and the first size above the limit."""
+    H = random_csr(n, min(7, n // 3 + 1), seed=n + s, empty_every=9)
+    V = workloads.start_block(n, s, seed=K)
+    rad = np.zeros(n)
+    np.add.at(rad, np.repeat(np.arange(n), np.diff(H.row_ptr)), np.abs(H.val))
+    a, b = 0.2, 1.05 * float(rad.max()) + 0.5
+    coeffs = cheb.filter_coeffs(0.1, K)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    ham = ham_from_oracle(P, H)
+    W = torch.full((n, s), float("nan"), dtype=torch.float64, device="cuda")
+    work = torch.full((2 * n * s,), float("nan"), dtype=torch.float64, device="cuda")
+    P.polfed_filter_apply(ham, a, b, coeffs, s, dev(V), W, work)
+    got = W.cpu().numpy()
+    assert np.linalg.norm(got - want) <= 1e-9 * np.linalg.norm(want)
+
+
 @pytest.mark.parametrize("s", (1, 8, 32))
 def test_fused_step_in_place_over_z(P, s):
     H = random_csr(513, 11, seed=3)
