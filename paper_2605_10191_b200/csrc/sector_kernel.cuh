@@ -99,8 +99,10 @@ struct RowOp {
   template <int... A>
   static __device__ __forceinline__ double apply(const double (&x)[N], double t1, double t2,
                                                  double acc, std::integer_sequence<int, A...>) {
+    double acc2 = 0.0;  // two chains: the bonds (A, A+1) and (A, A+2)
     (nn<A>(x, t1, acc), ...);
-    (nnn<A>(x, t2, acc), ...);
+    (nnn<A>(x, t2, acc2), ...);
+    if constexpr (NNN) acc += acc2;
     return acc;
   }
 };
