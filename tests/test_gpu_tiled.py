@@ -287,3 +287,35 @@ def test_tiled_full_size_config5_sampled_rows(P, fmt):
     P.polfed_fused_step(ham, s, 1.0 / b, -a / b, -1.0, c[0], B1, B2, V, B2)          # W
     diff = float((B2 - W).norm() / W.norm())
     assert diff <= 1e-13
+
+
+@pytest.mark.parametrize("fmt", FORMATS)
+def test_tiled_full_size_config5_long_pipeline_against_csr(P, fmt):
+    """Config 5 at full size (D = 10 400 600, s = 32), K = 40 with exact zeros among the
+    coefficients (the launches that skip the V read, R22): the dependency closure of a row is too
+    large for the oracle at this depth, so the whole block is compared with the CSR kernel, which
+    test_gpu_parity.py checks row by row against the oracle at this size."""
+    w = workloads.make_workload(5)
+    ham = build(P, w.n_sites, w.n_up, w.terms, fmt)
+    n, s, K = ham.n, w.s, 40
+    gen = torch.Generator(device="cuda").manual_seed(5140)
+    V = torch.randn(n, s, dtype=torch.float64, device="cuda", generator=gen)
+    a, b = 0.3, 17.0
+    c = np.random.default_rng(540).standard_normal(K + 1)
+    c[[1, 20, 21, 39]] = 0.0
+    work = torch.empty(P.polfed_filter_workspace_bytes_ham(ham, s) // 8, dtype=torch.float64,
+                       device="cuda")
+    W = torch.full((n, s), float("nan"), dtype=torch.float64, device="cuda")
+    P.polfed_filter_apply(ham, a, b, c, s, V, W, work)
+    torch.cuda.synchronize()
+    del work
+    # the same recurrence with the CSR kernel (Eq. 51; two rotating blocks)
+    B1 = c[K] * V
+    B2 = torch.empty_like(V)
+    for k in range(K - 1, 0, -1):
+        P.polfed_fused_step(ham, s, 2.0 / b, -2.0 * a / b, 0.0 if k == K - 1 else -1.0, c[k], B1,
+                            None if k == K - 1 else B2, V if c[k] != 0.0 else None, B2)
+        B1, B2 = B2, B1
+    P.polfed_fused_step(ham, s, 1.0 / b, -a / b, -1.0, c[0], B1, B2, V, B2)
+    assert bool(torch.isfinite(W).all())
+    assert float((B2 - W).abs().max()) <= 1e-12 * float(B2.abs().max())
