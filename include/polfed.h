@@ -199,8 +199,9 @@ size_t polfed_filter_workspace_bytes_ham(const polfed_ham* ham, int s);
  * b > 0 required (POLFED_ERANGE).  Enqueued on `stream`; allocates nothing; does not
  * synchronise.  On a POLFED_FORMAT_TILED or _SECTOR handle with s in {16, 32} the same recurrence
  * runs as K + 1 launches of the sweep kernel (see POLFED_FORMAT_TILED).  On a CSR handle with
- * n * s <= 4096 (config 1: a fused launch is far shorter than the launch latency) the K steps
- * run inside one persistent single-CTA kernel per 384 steps, both blocks in shared memory. */
+ * n * s <= 262144 (configs 1 and 2: a fused launch is far shorter than the launch latency) the K
+ * steps run inside one persistent kernel per 384 steps: a single CTA with both blocks in shared
+ * memory for n * s <= 4096, else a cooperative grid with a grid barrier between the steps. */
 int polfed_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,
                         int s, const double* d_V, double* d_W, void* d_work, void* stream);
 

@@ -61,7 +61,7 @@ int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const 
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   h->sm_count = sms > 0 ? sms : 148;
   cudaGetLastError();
-  if (n <= 4096) {  // only the persistent tiny-matrix filter asks for it
+  if (n <= 262144) {  // only the persistent small-matrix filter asks for it
     int rc = polfed::csr_max_row_len(n, d_row_ptr, &h->max_row_len);
     if (rc) {
       delete h;

@@ -74,8 +74,8 @@ bool flip_supports(const polfed_ham* ham, int s);
 int flip_step(const polfed_ham* ham, int s, double p, double q, double r, double c, const double* X,
               const double* Z, const double* V, double* Y, cudaStream_t st);
 
-// small_filter.cu: the whole recurrence in one persistent single-CTA kernel (n * s <= 4096).
-// small_filter_apply returns POLFED_ERANGE when the rows do not fit its shared memory.
+// small_filter.cu: the whole recurrence in one persistent kernel (n * s <= 262144).
+// small_filter_apply returns POLFED_ERANGE when it cannot take the matrix (caller: single launches).
 bool small_filter_supports(const polfed_ham* ham, int s);
 int csr_max_row_len(long long n, const int32_t* d_row_ptr, int* out);
 int small_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,

@@ -1,17 +1,20 @@
-// The whole Clenshaw recurrence of Eq. (51) PAPER.md:427-431 in ONE persistent kernel for tiny
-// matrices (BASELINE config 1: n * s <= 4096; a fused launch moves 0.02 us of memory traffic
-// against 5 us of launch latency; SURVEY section 7 "tiny configs are latency-bound").  One CTA
-// keeps both auxiliary blocks in shared memory for all K steps: every thread owns a few
-// (row, column) items and keeps its own entries of b_{k+1}, b_{k+2} and V in registers, the CSR
-// entries of its rows are staged in shared memory once per launch, a CTA barrier separates the
-// steps and the blocks rotate by a pointer swap inside the kernel (Fig. 5).  The coefficients
-// travel as kernel parameters, up to kSmallChunk recurrence steps per launch, so nothing is
-// allocated and no device buffer beyond the caller's two-block workspace is needed.
-// (A cooperative multi-CTA variant with a grid barrier per step was measured on config 2 and
-// lost to single launches: 9.8 against 6.1 us per product.)
+// The whole Clenshaw recurrence of Eq. (51) PAPER.md:427-431 in ONE persistent kernel for small
+// matrices (BASELINE configs 1 and 2: a fused launch moves 0.02-0.7 us of memory traffic against
+// 5-6 us of launch latency; SURVEY section 7 "tiny configs are latency-bound").  Every thread owns
+// a few (row, column) items and keeps its own entries of b_{k+1}, b_{k+2} and V in registers; the
+// CSR entries of its rows are staged in shared memory once per launch; the blocks rotate by a
+// pointer swap inside the kernel (Fig. 5).  n * s <= 4096: one CTA, both blocks in shared memory,
+// __syncthreads between the steps.  n * s <= 262144: a cooperative grid (one CTA per SM), blocks
+// in L2, a grid barrier between the steps.  The coefficients travel as kernel parameters, up to
+// kSmallChunk recurrence steps per launch, so nothing is allocated and no device buffer beyond the
+// caller's two-block workspace is needed.  DESIGN.md section 5e.
+#include <cooperative_groups.h>
+
 #include <algorithm>
 
 #include "common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace polfed {
 namespace {
@@ -36,14 +39,19 @@ struct SmallArgs {
 
 constexpr int kSingleItems = 4096;    // single-CTA variant: both blocks in shared memory
 constexpr int kSingleThreads = 1024;  // up to 4 items per thread
+constexpr int kGridThreads = 512;     // cooperative variant
+constexpr int kGridItems = 262144;    // n * s limit of the cooperative variant (config 2: 102 960)
 
 // Every thread owns the items it = tid + j * n_threads for the whole recurrence, so its own
 // entries of b_{k+1}, b_{k+2} and V stay in registers, and the CSR entries of its rows are staged
 // once per launch in shared memory ([entry][row slot]: the s threads of a row share a slot).  Per
 // step it gathers b_{k+1} at its row's columns from shared memory and publishes b_k there.
-template <int J>
-__global__ void __launch_bounds__(kSingleThreads) small_filter_kernel(const SmallArgs a) {
-  constexpr bool SINGLE = true;
+// SINGLE: one CTA, both blocks in shared memory, __syncthreads between the steps.  Otherwise a
+// cooperative grid of at most one CTA per SM: blocks in global memory (L2), a grid barrier
+// between the steps.
+template <bool SINGLE, int J>
+__global__ void __launch_bounds__(SINGLE ? kSingleThreads : kGridThreads)
+    small_filter_kernel(const SmallArgs a) {
   extern __shared__ double s_dyn[];
   const int tid = blockIdx.x * blockDim.x + threadIdx.x;
   const int n_threads = gridDim.x * blockDim.x;
@@ -99,9 +107,23 @@ __global__ void __launch_bounds__(kSingleThreads) small_filter_kernel(const Smal
       const int* ec = ent_col + j * rows_per_j + slot0;
       const double* xc = cur + col_j[j];
       double acc = 0.0;
+      if (SINGLE) {
 #pragma unroll 4
-      for (int k = 0; k < len[j]; ++k)
-        acc = fma(ev[k * slots], SINGLE ? xc[ec[k * slots]] : __ldcg(xc + ec[k * slots]), acc);
+        for (int k = 0; k < len[j]; ++k) acc = fma(ev[k * slots], xc[ec[k * slots]], acc);
+      } else {
+        // gathers from L2: ten independent loads in flight per round
+        for (int k0 = 0; k0 < len[j]; k0 += 10) {
+          double v[10], x[10];
+#pragma unroll
+          for (int u = 0; u < 10; ++u) {
+            const bool on = k0 + u < len[j];
+            v[u] = on ? ev[(k0 + u) * slots] : 0.0;
+            x[u] = on ? __ldcg(xc + ec[(k0 + u) * slots]) : 0.0;
+          }
+#pragma unroll
+          for (int u = 0; u < 10; ++u) acc = fma(v[u], x[u], acc);
+        }
+      }
       if (it < items) {
         double y = fma(p, acc, q * x_own[j]);
         y = fma(r, z_own[j], y);
@@ -116,7 +138,8 @@ __global__ void __launch_bounds__(kSingleThreads) small_filter_kernel(const Smal
     cur = old;
     old = t;
     if (i + 1 < a.n_steps) {
-      __syncthreads();
+      if (SINGLE) __syncthreads();
+      else cg::this_grid().sync();
     }
   }
   if (SINGLE && !a.last_is_w) {
@@ -143,16 +166,18 @@ __global__ void __launch_bounds__(256) max_row_len_kernel(long long n, const int
   if ((threadIdx.x & 31) == 0) atomicMax(out, v);
 }
 
-const void* const kKernels[4] = {
-    (const void*)small_filter_kernel<1>, (const void*)small_filter_kernel<2>,
-    (const void*)small_filter_kernel<4>, (const void*)small_filter_kernel<8>};
+const void* const kKernels[8] = {
+    (const void*)small_filter_kernel<true, 1>,  (const void*)small_filter_kernel<true, 2>,
+    (const void*)small_filter_kernel<true, 4>,  (const void*)small_filter_kernel<true, 8>,
+    (const void*)small_filter_kernel<false, 1>, (const void*)small_filter_kernel<false, 2>,
+    (const void*)small_filter_kernel<false, 4>, (const void*)small_filter_kernel<false, 8>};
 
 }  // namespace
 
 // True when the persistent kernel takes the recurrence of this handle and block size.
 bool small_filter_supports(const polfed_ham* ham, int s) {
   if (!ham || ham->tiled || ham->flip || ham->max_row_len < 1) return false;
-  return ham->n * (long long)s <= kSingleItems;
+  return ham->n * (long long)s <= kGridItems;
 }
 
 // Longest row of a CSR matrix (polfed_ham_from_csr records it in the handle).  Synchronises.
@@ -173,21 +198,27 @@ int csr_max_row_len(long long n, const int32_t* d_row_ptr, int* out) {
 int small_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const double* c, int s,
                        const double* d_V, double* d_W, double* cur, double* old, cudaStream_t st) {
   constexpr int kSmemCap = 200 * 1024;
-  static bool configured = false;
-  if (!configured) {
-    for (int v = 0; v < 4; ++v)
+  static int coop = -1;
+  if (coop < 0) {
+    int dev = 0;
+    POLFED_CUDA(cudaGetDevice(&dev));
+    POLFED_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    for (int v = 0; v < 8; ++v)
       POLFED_CUDA(cudaFuncSetAttribute(kKernels[v], cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        kSmemCap));
-    configured = true;
   }
   const int items = (int)ham->n * s;
-  const int j_used = (items + kSingleThreads - 1) / kSingleThreads;
+  const bool single = items <= kSingleItems;
+  if (!single && !coop) return POLFED_ERANGE;  // caller: single launches
+  const int threads = single ? kSingleThreads : kGridThreads;
+  const int grid = single ? 1 : std::min((items + kGridThreads - 1) / kGridThreads, ham->sm_count);
+  const int j_used = (items + grid * threads - 1) / (grid * threads);
   int jlog = 0;  // items per thread of the instantiation: 1, 2, 4 or 8
   while ((1 << jlog) < j_used) ++jlog;
-  const size_t smem = 2 * (size_t)items * sizeof(double) +
-                      ((size_t)1 << jlog) * (kSingleThreads / s) * ham->max_row_len * 12 + 16;
+  const size_t smem = (single ? 2 * (size_t)items * sizeof(double) : 0) +
+                      ((size_t)1 << jlog) * (threads / s) * ham->max_row_len * 12 + 16;
   if (jlog > 3 || smem > (size_t)kSmemCap) return POLFED_ERANGE;  // caller: single launches
-  const void* kernel = kKernels[jlog];
+  const void* kernel = kKernels[(single ? 0 : 4) + jlog];
 
   SmallArgs args{};
   args.n = (int)ham->n;
@@ -209,7 +240,11 @@ int small_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
     args.last_is_w = (k - n_steps + 1 == 0);
     for (int i = 0; i < n_steps; ++i) args.c[i] = c[k - i];
     void* params[] = {&args};
-    POLFED_CUDA(cudaLaunchKernel(kernel, dim3(1), dim3(kSingleThreads), params, smem, st));
+    if (single)
+      POLFED_CUDA(cudaLaunchKernel(kernel, dim3(1), dim3(kSingleThreads), params, smem, st));
+    else
+      POLFED_CUDA(cudaLaunchCooperativeKernel(kernel, dim3((unsigned)grid), dim3(kGridThreads), params,
+                                              smem, st));
     if (n_steps & 1) std::swap(cur, old);  // the kernel's rotation, seen from the host
     k -= n_steps;
   }
