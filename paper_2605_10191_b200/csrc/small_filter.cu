@@ -158,6 +158,93 @@ __global__ void __launch_bounds__(SINGLE ? kSingleThreads : kGridThreads)
   }
 }
 
+// Register variant for the smallest matrices (config 1: 924 rows, s = 1): rows of at most ML
+// entries, at most J items per thread -- the entries themselves (value and the element offset of
+// the gathered entry of b_{k+1}) stay in registers for the whole recurrence, padded with zero
+// values, so a step is ML independent shared-memory gathers and two FMA chains per item with no
+// loop, no entry loads and no length test.  One CTA, both blocks in shared memory.
+constexpr int kRegThreads = 512;
+constexpr int kRegMaxLen = 16;
+
+template <int J, int ML>
+__global__ void __launch_bounds__(kRegThreads) small_reg_kernel(const SmallArgs a) {
+  extern __shared__ double s_dyn[];
+  const int tid = threadIdx.x;
+  const int items = a.n * a.s;
+  double ev[J][ML];
+  int ec[J][ML];
+  double x_own[J], z_own[J], v_own[J];
+#pragma unroll
+  for (int j = 0; j < J; ++j) {
+    const int it = tid + j * kRegThreads;
+    const bool valid = it < items;
+    const int safe = valid ? it : 0;
+    const int row = safe / a.s, colj = safe - row * a.s;
+    const int e0 = __ldg(a.row_ptr + row);
+    const int len = valid ? __ldg(a.row_ptr + row + 1) - e0 : 0;
+#pragma unroll
+    for (int k = 0; k < ML; ++k) {
+      const bool on = k < len;
+      ev[j][k] = on ? __ldg(a.val + e0 + k) : 0.0;
+      ec[j][k] = on ? __ldg(a.col + e0 + k) * a.s + colj : safe;
+    }
+    x_own[j] = valid ? __ldcg(a.cur + it) : 0.0;
+    z_own[j] = (valid && a.first_has_z) ? __ldcg(a.old + it) : 0.0;
+    v_own[j] = valid ? __ldg(a.V + it) : 0.0;
+  }
+  double* cur = s_dyn;
+  double* old = s_dyn + items;
+#pragma unroll
+  for (int j = 0; j < J; ++j)
+    if (tid + j * kRegThreads < items) cur[tid + j * kRegThreads] = x_own[j];
+  __syncthreads();
+  const double p2 = 2.0 / a.b, q2 = -2.0 * a.a / a.b;
+  for (int i = 0; i < a.n_steps; ++i) {
+    const bool last = a.last_is_w && i + 1 == a.n_steps;
+    const double p = last ? 0.5 * p2 : p2, q = last ? 0.5 * q2 : q2;
+    const double r = (i == 0 && !a.first_has_z) ? 0.0 : -1.0;
+    const double c = a.c[i];
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const int it = tid + j * kRegThreads;
+      double x[ML];
+#pragma unroll
+      for (int k = 0; k < ML; ++k) x[k] = cur[ec[j][k]];
+      double acc0 = 0.0, acc1 = 0.0;
+#pragma unroll
+      for (int k = 0; k < ML; k += 2) {
+        acc0 = fma(ev[j][k], x[k], acc0);
+        acc1 = fma(ev[j][k + 1], x[k + 1], acc1);
+      }
+      double y = fma(p, acc0 + acc1, q * x_own[j]);
+      y = fma(r, z_own[j], y);
+      y = fma(c, v_own[j], y);
+      if (it < items) {
+        if (last) a.W[it] = y;
+        else old[it] = y;
+      }
+      z_own[j] = x_own[j];
+      x_own[j] = y;
+    }
+    double* t = cur;
+    cur = old;
+    old = t;
+    if (i + 1 < a.n_steps) __syncthreads();
+  }
+  if (!a.last_is_w) {  // more launches follow (see small_filter_kernel)
+    double* g_cur = (a.n_steps & 1) ? a.old : a.cur;
+    double* g_old = (a.n_steps & 1) ? a.cur : a.old;
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const int it = tid + j * kRegThreads;
+      if (it < items) {
+        g_cur[it] = x_own[j];
+        g_old[it] = z_own[j];
+      }
+    }
+  }
+}
+
 __global__ void __launch_bounds__(256) max_row_len_kernel(long long n, const int32_t* __restrict__ rp,
                                                           int* out) {
   const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -171,6 +258,8 @@ const void* const kKernels[8] = {
     (const void*)small_filter_kernel<true, 4>,  (const void*)small_filter_kernel<true, 8>,
     (const void*)small_filter_kernel<false, 1>, (const void*)small_filter_kernel<false, 2>,
     (const void*)small_filter_kernel<false, 4>, (const void*)small_filter_kernel<false, 8>};
+const void* const kRegKernels[2] = {(const void*)small_reg_kernel<1, kRegMaxLen>,
+                                    (const void*)small_reg_kernel<2, kRegMaxLen>};
 
 }  // namespace
 
@@ -209,6 +298,7 @@ int small_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
   }
   const int items = (int)ham->n * s;
   const bool single = items <= kSingleItems;
+  const bool in_regs = items <= 2 * kRegThreads && ham->max_row_len <= kRegMaxLen;
   if (!single && !coop) return POLFED_ERANGE;  // caller: single launches
   const int threads = single ? kSingleThreads : kGridThreads;
   const int grid = single ? 1 : std::min((items + kGridThreads - 1) / kGridThreads, ham->sm_count);
@@ -219,6 +309,7 @@ int small_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
                       ((size_t)1 << jlog) * (threads / s) * ham->max_row_len * 12 + 16;
   if (jlog > 3 || smem > (size_t)kSmemCap) return POLFED_ERANGE;  // caller: single launches
   const void* kernel = kKernels[(single ? 0 : 4) + jlog];
+  if (in_regs) kernel = kRegKernels[items > kRegThreads];
 
   SmallArgs args{};
   args.n = (int)ham->n;
@@ -240,7 +331,10 @@ int small_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
     args.last_is_w = (k - n_steps + 1 == 0);
     for (int i = 0; i < n_steps; ++i) args.c[i] = c[k - i];
     void* params[] = {&args};
-    if (single)
+    if (in_regs)
+      POLFED_CUDA(cudaLaunchKernel(kernel, dim3(1), dim3(kRegThreads), params,
+                                   2 * (size_t)items * sizeof(double), st));
+    else if (single)
       POLFED_CUDA(cudaLaunchKernel(kernel, dim3(1), dim3(kSingleThreads), params, smem, st));
     else
       POLFED_CUDA(cudaLaunchCooperativeKernel(kernel, dim3((unsigned)grid), dim3(kGridThreads), params,

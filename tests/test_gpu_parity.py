@@ -176,12 +176,15 @@ def test_fused_step_on_matrices_with_few_off_diagonal_values(P, s, values):
     assert np.all(np.abs(Y.cpu().numpy() - want) <= 1e-13 * (mag + 1e-300))
 
 
-@pytest.mark.parametrize("n,s,K", [(924, 1, 1000), (1, 1, 5), (300, 8, 385), (513, 4, 384), (4096, 1, 769),
-                                   (128, 32, 50), (4097, 1, 40)])
-def test_filter_on_tiny_matrices_persistent_kernel(P, n, s, K):
+@pytest.mark.parametrize("n,s,K,avg", [(924, 1, 1000, 7), (1, 1, 5, 7), (300, 8, 385, 7), (513, 4, 384, 7),
+                                       (4096, 1, 769, 7), (128, 32, 50, 7), (4097, 1, 40, 7),
+                                       # rows of at most 16 entries and n * s <= 1024: entries in registers
+                                       (924, 1, 1000, 3), (1000, 1, 385, 3), (512, 2, 30, 3), (100, 4, 40, 2),
+                                       (1024, 1, 3, 3), (1025, 1, 3, 3)])
+def test_filter_on_tiny_matrices_persistent_kernel(P, n, s, K, avg):
     """n * s <= 4096 runs all K steps inside one persistent kernel per 384 steps
     (csrc/small_filter.cu); orders that straddle the chunk size and the first size above the limit."""
-    H = random_csr(n, min(7, n // 3 + 1), seed=n + s, empty_every=9)
+    H = random_csr(n, min(avg, n // 3 + 1), seed=n + s, empty_every=9)
     V = workloads.start_block(n, s, seed=K)
     rad = np.zeros(n)
     np.add.at(rad, np.repeat(np.arange(n), np.diff(H.row_ptr)), np.abs(H.val))
