@@ -57,7 +57,7 @@ def gershgorin(H):
     return float(rad.max())
 
 
-FERMION = [(8, 4), (12, 6), (12, 3), (13, 6), (14, 9), (16, 8)]
+FERMION = [(8, 4), (9, 4), (10, 5), (12, 6), (12, 3), (13, 6), (14, 9), (16, 8)]
 
 
 @pytest.mark.parametrize("fmt", FORMATS)
@@ -78,8 +78,8 @@ def test_tiled_filter_random_coefficients(P, L, n_up, s, K, fmt):
 
 
 @pytest.mark.parametrize("fmt", FORMATS)
-@pytest.mark.parametrize("config,L_override,K", [(5, 16, 200), (5, 18, 1000), (3, 14, 600),
-                                                 (3, 16, None)])
+@pytest.mark.parametrize("config,L_override,K", [(5, 16, 200), (5, 18, 1000), (3, 12, 100),
+                                                 (3, 14, 600), (3, 16, None)])
 def test_tiled_filter_matches_oracle_on_workloads(P, config, L_override, K, fmt):
     w = workloads.make_workload(config, L_override=L_override)
     _, H = core.hamiltonian(w)
