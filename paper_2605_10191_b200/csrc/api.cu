@@ -1,4 +1,5 @@
 // Error reporting, handle lifetime and the CSR wrapper entry points of libpolfed.
+#include <mutex>
 #include <new>
 
 #include "common.cuh"
@@ -25,6 +26,34 @@ int fail(int code, const char* fmt, ...) {
   va_end(ap);
   g_error = buf;
   return code;
+}
+
+cudaError_t scratch_alloc(void** p, size_t bytes, cudaStream_t st) {
+  constexpr int kMaxDev = 64;
+  static std::mutex mu;
+  static cudaMemPool_t pools[kMaxDev] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDev) return cudaErrorInvalidDevice;
+  cudaMemPool_t pool;
+  {
+    std::lock_guard<std::mutex> lock(mu);
+    if (!pools[dev]) {
+      cudaMemPoolProps props{};
+      props.allocType = cudaMemAllocationTypePinned;
+      props.handleTypes = cudaMemHandleTypeNone;
+      props.location.type = cudaMemLocationTypeDevice;
+      props.location.id = dev;
+      e = cudaMemPoolCreate(&pools[dev], &props);
+      if (e != cudaSuccess) return e;
+      unsigned long long keep = ~0ull;
+      e = cudaMemPoolSetAttribute(pools[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+      if (e != cudaSuccess) return e;
+    }
+    pool = pools[dev];
+  }
+  return cudaMallocFromPoolAsync(p, bytes ? bytes : 1, pool, st);
 }
 
 }  // namespace polfed

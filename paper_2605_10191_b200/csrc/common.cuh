@@ -82,6 +82,11 @@ int small_filter_apply(const polfed_ham* ham, double a, double b, int K, const d
                        int s, const double* d_V, double* d_W, double* cur, double* old,
                        cudaStream_t st);
 
+// api.cu: stream-ordered scratch from the library's own memory pool of the current device (one per
+// device, created on first use, never trimmed: after the first call of a given size an
+// allocation is a free-list hit, not a mapping).  Free with cudaFreeAsync.
+cudaError_t scratch_alloc(void** p, size_t bytes, cudaStream_t st);
+
 // spmm_clenshaw.cu: the fused step without argument validation (flip handles: flip_step).
 int dispatch_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
                   const double* X, const double* Z, const double* V, double* Y, cudaStream_t st);

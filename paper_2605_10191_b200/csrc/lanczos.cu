@@ -79,30 +79,33 @@ struct DenseEigh {
   ~DenseEigh() {
     if (handle) cusolverDnDestroy(handle);
   }
-  // h_A: m x m symmetric (row- or column-major alike).  On return h_w ascending, h_Z column j =
-  // eigenvector j, stored contiguously (h_Z[j*m + i]).
-  int solve(int m, const double* h_A, double* h_w, double* h_Z, cudaStream_t st) {
+  // Device buffers for problems up to m x m.  Allocated once per solve of the library (cudaMalloc
+  // and cudaFree between the block steps cost up to a second each on a busy context).
+  int reserve(int m) {
     if (!handle) {
       if (cusolverDnCreate(&handle) != CUSOLVER_STATUS_SUCCESS)
         return fail(POLFED_ECUDA, "cusolverDnCreate failed");
     }
+    if ((size_t)m <= cap_m) return POLFED_OK;
+    cudaFree(A.p); cudaFree(w.p); cudaFree(work.p); cudaFree(info.p);
+    A.p = w.p = work.p = info.p = nullptr;
+    cap_m = 0;
+    POLFED_CUDA(A.alloc(sizeof(double) * (size_t)m * m));
+    POLFED_CUDA(w.alloc(sizeof(double) * (size_t)m));
+    POLFED_CUDA(info.alloc(sizeof(int)));
+    if (cusolverDnDsyevd_bufferSize(handle, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, m,
+                                    A.f64(), m, w.f64(), &lwork) != CUSOLVER_STATUS_SUCCESS)
+      return fail(POLFED_ECUDA, "cusolverDnDsyevd_bufferSize failed");
+    POLFED_CUDA(work.alloc(sizeof(double) * (size_t)lwork));
+    cap_m = (size_t)m;
+    return POLFED_OK;
+  }
+  // h_A: m x m symmetric (row- or column-major alike).  On return h_w ascending, h_Z column j =
+  // eigenvector j, stored contiguously (h_Z[j*m + i]).
+  int solve(int m, const double* h_A, double* h_w, double* h_Z, cudaStream_t st) {
+    int rc = reserve(m);
+    if (rc) return rc;
     cusolverDnSetStream(handle, st);
-    if ((size_t)m > cap_m) {
-      cudaFree(A.p); cudaFree(w.p); cudaFree(work.p); cudaFree(info.p);
-      A.p = w.p = work.p = info.p = nullptr;
-      POLFED_CUDA(A.alloc(sizeof(double) * (size_t)m * m));
-      POLFED_CUDA(w.alloc(sizeof(double) * (size_t)m));
-      POLFED_CUDA(info.alloc(sizeof(int)));
-      if (cusolverDnDsyevd_bufferSize(handle, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, m,
-                                      A.f64(), m, w.f64(), &lwork) != CUSOLVER_STATUS_SUCCESS)
-        return fail(POLFED_ECUDA, "cusolverDnDsyevd_bufferSize failed");
-      POLFED_CUDA(work.alloc(sizeof(double) * (size_t)lwork));
-      cap_m = (size_t)m;
-    } else {
-      if (cusolverDnDsyevd_bufferSize(handle, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, m,
-                                      A.f64(), m, w.f64(), &lwork) != CUSOLVER_STATUS_SUCCESS)
-        return fail(POLFED_ECUDA, "cusolverDnDsyevd_bufferSize failed");
-    }
     POLFED_CUDA(cudaMemcpyAsync(A.p, h_A, sizeof(double) * (size_t)m * m, cudaMemcpyHostToDevice, st));
     if (cusolverDnDsyevd(handle, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, m, A.f64(), m,
                          w.f64(), work.f64(), lwork, static_cast<int*>(info.p)) != CUSOLVER_STATUS_SUCCESS)
@@ -408,6 +411,8 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
   rc = qr.init();
   if (rc) return rc;
   DenseEigh eig;
+  rc = eig.reserve((int)std::max<long long>(m_cap, wp));
+  if (rc) return rc;
 
   std::vector<double> HL((size_t)m_cap * m_cap, 0.0);  // H_L, preallocated
   std::vector<double> hC((size_t)(m_cap + s) * s), Bk(s * s), Bprev(s * s, 0.0);

@@ -400,19 +400,11 @@ int polfed_filter_apply_host(const polfed_ham* ham, double a, double b, int K,
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const size_t bytes = (size_t)ham->n * s * sizeof(double);
   const size_t pitch = (bytes + 127) / 128 * 128;  // every sub-buffer starts on a 128-byte boundary
-  // V | W | work from the stream-ordered pool: after the first call the blocks are reused, not
-  // allocated (the pool keeps them: release threshold raised once per device)
-  {
-    int dev = 0;
-    POLFED_CUDA(cudaGetDevice(&dev));
-    cudaMemPool_t pool;
-    POLFED_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
-    unsigned long long keep = ~0ull;
-    POLFED_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-  }
+  // V | W | work from the library's stream-ordered pool: after the first call the blocks are
+  // reused, not allocated
   char* d_all = nullptr;
-  POLFED_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&d_all),
-                              2 * pitch + polfed_filter_workspace_bytes_ham(ham, s), st));
+  POLFED_CUDA(polfed::scratch_alloc(reinterpret_cast<void**>(&d_all),
+                                    2 * pitch + polfed_filter_workspace_bytes_ham(ham, s), st));
   double* d_V = reinterpret_cast<double*>(d_all);
   double* d_W = reinterpret_cast<double*>(d_all + pitch);
   void* d_work = d_all + 2 * pitch;

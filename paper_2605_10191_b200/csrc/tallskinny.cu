@@ -316,13 +316,13 @@ __global__ void __launch_bounds__(256) moments_kernel(long long n, const int32_t
   }
 }
 
-// Scratch for per-CTA partial results from the stream-ordered pool (reused after the first call).
+// Scratch for per-CTA partial results from the library's stream-ordered pool (common.cuh).
 struct PoolBuf {
   double* p = nullptr;
   cudaStream_t st;
   explicit PoolBuf(cudaStream_t s) : st(s) {}
   cudaError_t alloc(size_t doubles) {
-    return cudaMallocAsync(reinterpret_cast<void**>(&p), sizeof(double) * (doubles ? doubles : 1), st);
+    return scratch_alloc(reinterpret_cast<void**>(&p), sizeof(double) * doubles, st);
   }
   ~PoolBuf() {
     if (p) cudaFreeAsync(p, st);
