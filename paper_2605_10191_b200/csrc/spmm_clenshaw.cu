@@ -112,6 +112,11 @@ fused_step_kernel(int n, const int32_t* __restrict__ row_ptr, const int32_t* __r
   const long long cta_row0 = (long long)blockIdx.x * rows_per_cta;
   const int cta_row1 = (int)min((long long)n, cta_row0 + rows_per_cta);
 
+  // Programmatic dependent launch: the next step's CTAs may be scheduled while this grid drains;
+  // they load their row pointers and first entries (matrix data, never written) and then wait
+  // for this grid to complete before they touch a block.
+  asm volatile("griddepcontrol.launch_dependents;");
+  bool waited = false;
   for (int base = (int)cta_row0 + warp * RPW; base < cta_row1; base += kWarps * RPW) {
     const int row = base + sub;
     const bool active = row < cta_row1;
@@ -126,6 +131,10 @@ fused_step_kernel(int n, const int32_t* __restrict__ row_ptr, const int32_t* __r
 
     if constexpr (LPR == 1) {
       // one thread per row (S = 1, 2)
+      if (!waited) {
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+        waited = true;
+      }
       for (int e = e0; e < e1; ++e) {
         int cj = __ldcs(col + e);
         double vj;
@@ -142,13 +151,26 @@ fused_step_kernel(int n, const int32_t* __restrict__ row_ptr, const int32_t* __r
     } else {
       const int len = e1 - e0;
       const int maxlen = __reduce_max_sync(0xffffffffu, len);
+      // the entries of chunk i + 1 are loaded before the gathers of chunk i
+      int cc_n = 0;
+      double vv_n = 0.0;
+      if (e0 + sl < e1) {
+        cc_n = __ldcs(col + e0 + sl);
+        if constexpr (!PACKED) vv_n = __ldcs(val + e0 + sl);
+      }
+      if (!waited) {
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+        waited = true;
+      }
       for (int off = 0; off < maxlen; off += LPR) {
-        const int e = e0 + off + sl;
-        int cc = 0;
-        double vv = 0.0;
-        if (e < e1) {
-          cc = __ldcs(col + e);
-          if constexpr (!PACKED) vv = __ldcs(val + e);
+        const int cc = cc_n;
+        const double vv = vv_n;
+        const int en = e0 + off + LPR + sl;
+        cc_n = 0;
+        vv_n = 0.0;
+        if (en < e1) {
+          cc_n = __ldcs(col + en);
+          if constexpr (!PACKED) vv_n = __ldcs(val + en);
         }
         const int rem = len - off;  // entries of this row left in the chunk (may be <= 0)
 #pragma unroll
@@ -228,22 +250,35 @@ int launch_step_v(const polfed_ham* ham, double p, double q, double r, double c,
   if (pk)
     for (int i = 0; i < 16; ++i) vt.v[i] = pk->vals[i];
   const int nv = pk ? pk->n_vals : 0;
-#define POLFED_PK(UZ, UV, NV)                                                                    \
-  fused_step_kernel<S, VEC, UZ, UV, NV><<<grid, kThreads, 0, st>>>(                              \
-      n, pk->d_row_ptr, reinterpret_cast<const int32_t*>(pk->d_pcol), pk->d_diag, X, Z, V, Y, p, \
-      q, r, c, rows_per_cta, vt)
-#define POLFED_GO(UZ, UV)                                                                        \
-  if (nv == 1) POLFED_PK(UZ, UV, 1);                                                             \
-  else if (nv == 2) POLFED_PK(UZ, UV, 2);                                                        \
-  else                                                                                           \
-    fused_step_kernel<S, VEC, UZ, UV, 0><<<grid, kThreads, 0, st>>>(                             \
-        n, ham->d_row_ptr, ham->d_col, ham->d_val, X, Z, V, Y, p, q, r, c, rows_per_cta, vt)
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(kThreads);
+  cfg.stream = st;
+  cudaLaunchAttribute attr{};
+  attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr.val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = &attr;
+  cfg.numAttrs = 1;
+  const int32_t* pk_rp = pk ? pk->d_row_ptr : nullptr;
+  const int32_t* pk_col = pk ? reinterpret_cast<const int32_t*>(pk->d_pcol) : nullptr;
+  const double* pk_diag = pk ? pk->d_diag : nullptr;
+  cudaError_t le = cudaSuccess;
+#define POLFED_PK(UZ, UV, NV)                                                                     \
+  le = cudaLaunchKernelEx(&cfg, fused_step_kernel<S, VEC, UZ, UV, NV>, n, pk_rp, pk_col, pk_diag, \
+                          X, Z, V, Y, p, q, r, c, rows_per_cta, vt)
+#define POLFED_GO(UZ, UV)                                                                         \
+  if (nv == 1) POLFED_PK(UZ, UV, 1);                                                              \
+  else if (nv == 2) POLFED_PK(UZ, UV, 2);                                                         \
+  else                                                                                            \
+    le = cudaLaunchKernelEx(&cfg, fused_step_kernel<S, VEC, UZ, UV, 0>, n, ham->d_row_ptr,        \
+                            ham->d_col, ham->d_val, X, Z, V, Y, p, q, r, c, rows_per_cta, vt)
   if (uz && uv) { POLFED_GO(true, true); }
   else if (uz) { POLFED_GO(true, false); }
   else if (uv) { POLFED_GO(false, true); }
   else { POLFED_GO(false, false); }
 #undef POLFED_GO
 #undef POLFED_PK
+  if (le != cudaSuccess) return fail(POLFED_ECUDA, "fused_step_kernel: %s", cudaGetErrorString(le));
   POLFED_LAUNCH_CHECK("fused_step_kernel");
   return POLFED_OK;
 }
