@@ -21,9 +21,11 @@ namespace {
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 
-// VEC doubles per lane: 4 (256-bit accesses) for S >= 16 when every block is 32-byte aligned --
-// half the lanes per row, so half the quad shuffles per stored entry (a shuffle costs two LSU
-// cycles, a 128-byte gather one: profiles/r01_flip_config4.md) -- else 2, else 1.
+// VEC doubles per lane: 2 (128-bit accesses) for S >= 2.  Round 1 used 4 (256-bit accesses, half
+// the lanes per row, half the shuffles per entry) for S >= 16; with the packed entries and the
+// entry loads one chunk ahead the step is bound by latency, not by the shuffles, and twice the
+// entries per chunk win: config 3 24.1 -> 20.9 us, config 4 (CSR) 239 -> 229 us, config 5 (CSR)
+// 6.83 -> 6.64 ms; one double per lane loses everywhere (30.1 us, 331 us, 8.0 ms).
 template <int S, int VEC_>
 struct Shape {
   static constexpr int VEC = VEC_;
@@ -40,11 +42,7 @@ struct Acc {
 template <int VEC>
 __device__ __forceinline__ Acc<VEC> load_gather(const double* p) {  // X rows: keep in L1/L2
   Acc<VEC> a;
-  if constexpr (VEC == 4) {
-    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
-                 : "=d"(a.v[0]), "=d"(a.v[1]), "=d"(a.v[2]), "=d"(a.v[3])
-                 : "l"(p));
-  } else if constexpr (VEC == 2) {
+  if constexpr (VEC == 2) {
     double2 t = __ldg(reinterpret_cast<const double2*>(p));
     a.v[0] = t.x;
     a.v[1] = t.y;
@@ -57,11 +55,7 @@ __device__ __forceinline__ Acc<VEC> load_gather(const double* p) {  // X rows: k
 template <int VEC>
 __device__ __forceinline__ Acc<VEC> load_stream(const double* p) {  // Z, V: touched once
   Acc<VEC> a;
-  if constexpr (VEC == 4) {
-    asm volatile("ld.global.cs.v4.f64 {%0,%1,%2,%3}, [%4];"
-                 : "=d"(a.v[0]), "=d"(a.v[1]), "=d"(a.v[2]), "=d"(a.v[3])
-                 : "l"(p));
-  } else if constexpr (VEC == 2) {
+  if constexpr (VEC == 2) {
     double2 t = __ldcs(reinterpret_cast<const double2*>(p));
     a.v[0] = t.x;
     a.v[1] = t.y;
@@ -73,11 +67,7 @@ __device__ __forceinline__ Acc<VEC> load_stream(const double* p) {  // Z, V: tou
 
 template <int VEC>
 __device__ __forceinline__ void store_stream(double* p, const Acc<VEC>& a) {
-  if constexpr (VEC == 4) {
-    asm volatile("st.global.cs.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a.v[0]), "d"(a.v[1]),
-                 "d"(a.v[2]), "d"(a.v[3])
-                 : "memory");
-  } else if constexpr (VEC == 2) {
+  if constexpr (VEC == 2) {
     __stcs(reinterpret_cast<double2*>(p), make_double2(a.v[0], a.v[1]));
   } else {
     __stcs(p, a.v[0]);
@@ -283,15 +273,9 @@ int launch_step_v(const polfed_ham* ham, double p, double q, double r, double c,
   return POLFED_OK;
 }
 
-inline bool aligned32(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 31u) == 0; }
-
 template <int S>
 int launch_step(const polfed_ham* ham, double p, double q, double r, double c, const double* X,
                 const double* Z, const double* V, double* Y, cudaStream_t st) {
-  if constexpr (S >= 16) {
-    if (aligned32(X) && aligned32(Y) && (r == 0.0 || aligned32(Z)) && (c == 0.0 || aligned32(V)))
-      return launch_step_v<S, 4>(ham, p, q, r, c, X, Z, V, Y, st);
-  }
   return launch_step_v<S, (S >= 2) ? 2 : 1>(ham, p, q, r, c, X, Z, V, Y, st);
 }
 
