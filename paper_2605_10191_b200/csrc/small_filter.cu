@@ -39,7 +39,7 @@ struct SmallArgs {
 
 constexpr int kSingleItems = 4096;    // single-CTA variant: both blocks in shared memory
 constexpr int kSingleThreads = 1024;  // up to 4 items per thread
-constexpr int kGridThreads = 512;     // cooperative variant
+constexpr int kGridThreads = 512;     // cooperative variant (1024 when that saves a second item per thread)
 constexpr int kGridItems = 262144;    // n * s limit of the cooperative variant (config 2: 102 960)
 
 // Every thread owns the items it = tid + j * n_threads for the whole recurrence, so its own
@@ -50,7 +50,7 @@ constexpr int kGridItems = 262144;    // n * s limit of the cooperative variant 
 // cooperative grid of at most one CTA per SM: blocks in global memory (L2), a grid barrier
 // between the steps.
 template <bool SINGLE, int J>
-__global__ void __launch_bounds__(SINGLE ? kSingleThreads : kGridThreads)
+__global__ void __launch_bounds__(SINGLE ? kSingleThreads : 2 * kGridThreads)
     small_filter_kernel(const SmallArgs a) {
   extern __shared__ double s_dyn[];
   const int tid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -300,8 +300,10 @@ int small_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
   const bool single = items <= kSingleItems;
   const bool in_regs = items <= 2 * kRegThreads && ham->max_row_len <= kRegMaxLen;
   if (!single && !coop) return POLFED_ERANGE;  // caller: single launches
-  const int threads = single ? kSingleThreads : kGridThreads;
-  const int grid = single ? 1 : std::min((items + kGridThreads - 1) / kGridThreads, ham->sm_count);
+  // cooperative variant: 1024-thread CTAs when 512-thread CTAs would leave threads with two items
+  const int grid_threads = items > kGridThreads * ham->sm_count ? 2 * kGridThreads : kGridThreads;
+  const int threads = single ? kSingleThreads : grid_threads;
+  const int grid = single ? 1 : std::min((items + grid_threads - 1) / grid_threads, ham->sm_count);
   const int j_used = (items + grid * threads - 1) / (grid * threads);
   int jlog = 0;  // items per thread of the instantiation: 1, 2, 4 or 8
   while ((1 << jlog) < j_used) ++jlog;
@@ -337,8 +339,8 @@ int small_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
     else if (single)
       POLFED_CUDA(cudaLaunchKernel(kernel, dim3(1), dim3(kSingleThreads), params, smem, st));
     else
-      POLFED_CUDA(cudaLaunchCooperativeKernel(kernel, dim3((unsigned)grid), dim3(kGridThreads), params,
-                                              smem, st));
+      POLFED_CUDA(cudaLaunchCooperativeKernel(kernel, dim3((unsigned)grid), dim3((unsigned)threads),
+                                              params, smem, st));
     if (n_steps & 1) std::swap(cur, old);  // the kernel's rotation, seen from the host
     k -= n_steps;
   }
