@@ -205,10 +205,11 @@ size_t polfed_filter_workspace_bytes_ham(const polfed_ham* ham, int s);
 int polfed_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,
                         int s, const double* d_V, double* d_W, void* d_work, void* stream);
 
-/* Same operation on HOST blocks: takes device blocks from the device's stream-ordered memory
- * pool (cudaMallocAsync; the pool's release threshold is raised so that later calls reuse them
- * instead of allocating), copies h_V up, runs polfed_filter_apply, copies W down into h_W,
- * returns the blocks to the pool, synchronises.  The end-to-end entry. */
+/* Same operation on HOST blocks: takes device blocks from the library's own stream-ordered
+ * memory pool (one per device, created on first use and never trimmed, so that later calls
+ * reuse the blocks instead of allocating; the device's default pool is left alone), copies h_V
+ * up, runs polfed_filter_apply, copies W down into h_W, returns the blocks to the pool,
+ * synchronises.  The end-to-end entry. */
 int polfed_filter_apply_host(const polfed_ham* ham, double a, double b, int K,
                              const double* h_coeffs, int s, const double* h_V, double* h_W,
                              void* stream);
@@ -273,7 +274,8 @@ int polfed_kpm_dos(const double* h_moments, int n_moments, const double* e_resca
  * pointers DEVICE, 16-byte aligned.  Every sum runs in a fixed order (bit-reproducible).
  * variant: 0 = the library's choice (fp64 tensor-core mma for s >= 8), 1 = the shared-memory FMA
  * kernel, 2 = tensor cores (s >= 8 only, else the FMA kernel).  Enqueued on `stream`; scratch for
- * the per-CTA partial sums comes from the device's stream-ordered pool. */
+ * the per-CTA partial sums comes from the library's stream-ordered pool (see
+ * polfed_filter_apply_host). */
 int polfed_block_gram(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
                       const double* d_B, double* d_C, int variant, void* stream);
 int polfed_block_update(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
