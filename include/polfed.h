@@ -297,6 +297,12 @@ typedef struct {
   int32_t kpm_vectors;    /* KPM: columns R of d_kpm_block, a positive multiple of 4 (paper: 100) */
   const double* d_kpm_block; /* KPM: n x kpm_vectors row-major DEVICE block of iid zero-mean
                              unit-variance entries drawn by the caller (no RNG crosses the ABI) */
+  int32_t window_levels;  /* levels N the filter window of Eq. (40)-(41) is sized for.  <= 0: the
+                             paper's rule, N = nev ("contains exactly N_ev eigenvalues"),
+                             plus max(2, 10 %) (R4).  Larger N = lower order K; must be >= nev.
+                             Measured on config 3 (nev = 100, s = 16): the Krylov dimension that
+                             block Lanczos needs stays near 4.6 nev once the window holds <= 2 nev
+                             levels, so N = 2 nev halves K and the time */
 } polfed_options;
 enum { POLFED_DOS_GAUSSIAN = 0, POLFED_DOS_KPM = 1 };
 
@@ -310,7 +316,8 @@ typedef struct {
   double seconds_extraction, seconds_total;
   double rho_gaussian, rho_kpm;   /* states per unit rescaled energy at the target (0: not evaluated) */
   int32_t K_kpm;                  /* order the KPM density of states gives (0 if not evaluated) */
-  int32_t nev_window;             /* levels the filter window is sized for: nev + max(2, 10 %) */
+  int32_t nev_window;             /* levels the filter window is sized for: nev + max(2, 10 %), or
+                                     options->window_levels */
   double seconds_dos;             /* moments of the density-of-states estimate */
 } polfed_report;
 

@@ -52,7 +52,7 @@ class _Options(C.Structure):
                 ("K_override", C.c_int32), ("bounds_steps", C.c_int32),
                 ("bounds_margin", C.c_double), ("a", C.c_double), ("b", C.c_double),
                 ("sigma_is_rescaled", C.c_int32), ("dos", C.c_int32), ("kpm_moments", C.c_int32),
-                ("kpm_vectors", C.c_int32), ("d_kpm_block", C.c_void_p)]
+                ("kpm_vectors", C.c_int32), ("d_kpm_block", C.c_void_p), ("window_levels", C.c_int32)]
 
 
 class _Report(C.Structure):
@@ -427,13 +427,14 @@ def polfed_block_lanczos_eigs(ham: Ham, sigma: float, nev: int, s: int, V0, *, t
                               bounds_steps: int = 0, bounds_margin: float = -1.0, a: float = 0.0,
                               b: float = 0.0, sigma_is_rescaled: bool = False, stream=None,
                               allow_unconverged: bool = False, kpm_block=None,
-                              kpm_moments: int = 0):
+                              kpm_moments: int = 0, window_levels: int = 0):
     """The nev eigenpairs of H nearest sigma: (evals ndarray, evecs CUDA tensor n x nev,
     residuals ndarray, report dict).  Raises PolfedError(ENOCONV) unless allow_unconverged.
-    kpm_block (CUDA tensor n x R, R a multiple of 4): size K with the KPM density of states."""
+    kpm_block (CUDA tensor n x R, R a multiple of 4): size K with the KPM density of states.
+    window_levels > 0: size the filter window for that many levels instead of nev + 10 %."""
     import torch
     opt = _Options(tol, max_krylov_dim, check_every, K_override, bounds_steps, bounds_margin, a, b,
-                   int(bool(sigma_is_rescaled)), 0, 0, 0, None)
+                   int(bool(sigma_is_rescaled)), 0, 0, 0, None, int(window_levels))
     if kpm_block is not None:
         if (kpm_block.dim() != 2 or kpm_block.shape[0] != ham.n or kpm_block.dtype != torch.float64
                 or not kpm_block.is_cuda or not kpm_block.is_contiguous()):

@@ -311,7 +311,9 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
   // The window is sized for 10 % more levels than asked for (at least 2 more): a density estimate
   // that is a few per cent high would otherwise leave fewer than nev levels inside the main lobe
   // and secondary-peak levels would fill the set (reading R4).
-  const int nev_window = nev + std::max(2, (nev + 9) / 10);
+  if (opt.window_levels > 0 && opt.window_levels < nev)
+    return fail(POLFED_EINVAL, "polfed_block_lanczos_eigs: window_levels=%d < nev=%d", opt.window_levels, nev);
+  const int nev_window = opt.window_levels > 0 ? opt.window_levels : nev + std::max(2, (nev + 9) / 10);
   rep.nev_window = nev_window;
   int K = opt.K_override;
   double rho = 0.0;

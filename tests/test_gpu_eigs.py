@@ -115,6 +115,29 @@ def test_eigs_shrunk_workloads_residuals_and_completeness(P, config, L_override,
     assert np.max(np.abs(evals[1:-1] - nearest[1:-1])) <= 1e-9 * hnorm
 
 
+def test_eigs_wider_window_gives_lower_order_and_the_same_pairs(P):
+    """options.window_levels: the window of Eq. (40)-(41) sized for 2 nev levels instead of
+    nev + 10 % -- about half the order, the same nev pairs nearest the target (dense truth)."""
+    w = workloads.make_workload(2)
+    _, H = core.hamiltonian(w)
+    ev = np.linalg.eigvalsh(H.to_dense())
+    hnorm = max(abs(ev[0]), abs(ev[-1]))
+    V0 = dev(workloads.start_block(H.n, w.s, seed=2002, orthonormal=True))
+    ham = build(P, w)
+    _, _, _, rep0 = P.polfed_block_lanczos_eigs(ham, 0.0, w.nev, w.s, V0, sigma_is_rescaled=True)
+    evals, evecs, resid, rep = P.polfed_block_lanczos_eigs(ham, 0.0, w.nev, w.s, V0, sigma_is_rescaled=True,
+                                                           window_levels=2 * w.nev)
+    assert rep0["nev_window"] == w.nev + 5 and rep["nev_window"] == 2 * w.nev
+    assert 0.45 * rep0["K"] <= rep["K"] <= 0.65 * rep0["K"]
+    sigma = rep["a"] + rep["b"] * rep["lambda_rescaled"]
+    check_pairs(H, evals, evecs, resid, 1e-8 * hnorm)
+    nearest = np.sort(ev[np.argsort(np.abs(ev - sigma))[: w.nev]])
+    assert np.max(np.abs(evals[1:-1] - nearest[1:-1])) <= 1e-9 * hnorm
+    with pytest.raises(P.PolfedError) as err:
+        P.polfed_block_lanczos_eigs(ham, 0.0, w.nev, w.s, V0, sigma_is_rescaled=True, window_levels=w.nev - 1)
+    assert err.value.code == P.binding.EINVAL
+
+
 def test_eigs_reports_no_convergence_and_bad_arguments(P):
     w = workloads.make_workload(1)
     ham = build(P, w)
