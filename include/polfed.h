@@ -176,7 +176,11 @@ int polfed_ham_csr(const polfed_ham* ham, int64_t* n, int64_t* nnz, const int32_
  * d_Z is not read when r == 0 (may be NULL), d_V is not read when c == 0 (may be NULL).
  * d_Y may alias d_Z or d_V (row i of Z and V is read only by the threads that write row i
  * of Y); d_Y must not overlap d_X.  Also serves H X (p=1), Eq. (28)-(30) (KPM recurrence)
- * and the Lanczos three-term step.  Enqueued on `stream`; allocates nothing. */
+ * and the Lanczos three-term step.  Enqueued on `stream`; allocates nothing.  CSR handles launch
+ * it with programmatic stream serialisation: consecutive steps on one stream overlap the tail of
+ * one launch with the start of the next, which reads only the matrix arrays of the handle before
+ * the preceding kernel has completed and every block after (so the matrix arrays must not be
+ * written by work that is still in flight on `stream`). */
 int polfed_fused_step(const polfed_ham* ham, int s, double p, double q, double r, double c,
                       const double* d_X, const double* d_Z, const double* d_V, double* d_Y,
                       void* stream);
