@@ -409,11 +409,13 @@ def run_cuda(args):
             torch.cuda.empty_cache()
             warm_up_solver(P)
             line["seconds_to_nev"] = [time_to_nev(P, int(c)) for c in args.eigs.split(",") if c]
-            if "3" in args.eigs.split(","):
-                # the library's option for a wider filter window (include/polfed.h):
-                # config 3 again with the window sized for 2 nev levels, reported beside the
-                # paper's rule, not instead of it
-                line["seconds_to_nev_wide_window"] = [time_to_nev(P, 3, window_levels=200)]
+            # the library's option for a wider filter window (include/polfed.h):
+            # the solve again with the window sized for 2 nev levels, reported beside the
+            # paper's rule, not instead of it
+            wide = [int(c) for c in args.eigs_wide.split(",") if c and c in args.eigs.split(",")]
+            if wide:
+                line["seconds_to_nev_wide_window"] = [
+                    time_to_nev(P, c, window_levels=2 * workloads.make_workload(c).nev) for c in wide]
             line["seconds_to_nev_warmup"] = "one untimed solve of config 1 shrunk to L = 10 (loads cuSOLVER and the solver's kernels)"
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(args.config)
@@ -586,6 +588,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-reorth", action="store_true",
                     help="skip the timing of the reorthogonalisation products")
+    ap.add_argument("--eigs-wide", default="3",
+                    help="configs of --eigs that are solved a second time with window_levels = 2 nev")
     ap.add_argument("--eigs", default="1,2,3",
                     help="configs whose full eigen-solve is timed at N=1 ('' to skip; 4 takes minutes)")
     args = ap.parse_args()
