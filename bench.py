@@ -489,6 +489,9 @@ def hot_path_on_config(P, config: int, peak: float, fmt_name: str = ""):
             "filter_order": K, "filter_apply_ms": apply_ms,
             "filter_steps_per_s": K / (apply_ms * 1e-3),
             "us_per_product_in_filter": apply_ms * 1e3 / K,
+            # the same byte count over the time of one product inside polfed_filter_apply (for the
+            # small configs the single launches above are bound by the Python call, not the GPU)
+            "frac_of_measured_in_filter": by / (apply_ms * 1e-3 / K) / 1e9 / peak,
             "l2": "inputs exceed L2" if by > 4 * 126e6 else "working set fits L2 (not flushed)"}
 
 

@@ -49,6 +49,11 @@ typedef struct polfed_ham polfed_ham;
 const char* polfed_last_error(void);
 /* major*10000 + minor*100 + patch */
 int polfed_version(void);
+/* Returns the unused memory of the library's stream-ordered scratch pool on the current device
+ * to the driver (polfed_filter_apply_host and the eigen-solver keep their scratch blocks in that
+ * pool between calls, up to 6 blocks of n*s doubles, so that later calls do not allocate).
+ * Synchronises the device.  Safe to call at any time; the next call allocates again. */
+int polfed_release_scratch(void);
 
 /* ------------------------------------------------------------------------------------------
  * Basis (the paper uses symmetry sectors but never says how they are

@@ -5,7 +5,7 @@ The functions re-exported here are thin ctypes wrappers with the names of the C 
 """
 from .binding import (  # noqa: F401
     Basis, Ham, PolfedError, EXPORTS, LIB_PATH, TERM_KINDS, FORMAT_CSR, FORMAT_TILED, FORMAT_FLIP, FORMAT_SECTOR,
-    lib, polfed_last_error, polfed_version,
+    lib, polfed_last_error, polfed_version, polfed_release_scratch,
     polfed_build_basis, polfed_basis_dim, polfed_basis_states, polfed_basis_rank,
     polfed_build_hamiltonian, polfed_ham_from_csr, polfed_ham_csr,
     polfed_fused_step, polfed_filter_workspace_bytes, polfed_filter_workspace_bytes_ham,

@@ -20,7 +20,7 @@ TERM_KINDS = {"ZZ": 0, "Z": 1, "NN": 2, "N": 3, "EXCH": 4, "HOPJW": 5, "XX": 6}
 FORMAT_CSR, FORMAT_TILED, FORMAT_FLIP, FORMAT_SECTOR = 0, 2, 3, 4
 
 EXPORTS = (
-    "polfed_last_error", "polfed_version",
+    "polfed_last_error", "polfed_version", "polfed_release_scratch",
     "polfed_build_basis", "polfed_basis_destroy", "polfed_basis_dim", "polfed_basis_states",
     "polfed_basis_rank",
     "polfed_build_hamiltonian", "polfed_ham_from_csr", "polfed_ham_destroy", "polfed_ham_csr",
@@ -152,6 +152,11 @@ def polfed_last_error() -> str:
 
 def polfed_version() -> int:
     return int(lib().polfed_version())
+
+
+def polfed_release_scratch() -> None:
+    """Give the unused memory of the library's scratch pool back to the driver."""
+    _check(lib().polfed_release_scratch())
 
 
 # ---- basis ----------------------------------------------------------------------------

@@ -28,30 +28,33 @@ int fail(int code, const char* fmt, ...) {
   return code;
 }
 
+namespace {
+constexpr int kMaxDev = 64;
+std::mutex g_pool_mu;
+cudaMemPool_t g_pools[kMaxDev] = {};
+}  // namespace
+
 cudaError_t scratch_alloc(void** p, size_t bytes, cudaStream_t st) {
-  constexpr int kMaxDev = 64;
-  static std::mutex mu;
-  static cudaMemPool_t pools[kMaxDev] = {};
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if (dev < 0 || dev >= kMaxDev) return cudaErrorInvalidDevice;
   cudaMemPool_t pool;
   {
-    std::lock_guard<std::mutex> lock(mu);
-    if (!pools[dev]) {
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    if (!g_pools[dev]) {
       cudaMemPoolProps props{};
       props.allocType = cudaMemAllocationTypePinned;
       props.handleTypes = cudaMemHandleTypeNone;
       props.location.type = cudaMemLocationTypeDevice;
       props.location.id = dev;
-      e = cudaMemPoolCreate(&pools[dev], &props);
+      e = cudaMemPoolCreate(&g_pools[dev], &props);
       if (e != cudaSuccess) return e;
       unsigned long long keep = ~0ull;
-      e = cudaMemPoolSetAttribute(pools[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+      e = cudaMemPoolSetAttribute(g_pools[dev], cudaMemPoolAttrReleaseThreshold, &keep);
       if (e != cudaSuccess) return e;
     }
-    pool = pools[dev];
+    pool = g_pools[dev];
   }
   return cudaMallocFromPoolAsync(p, bytes ? bytes : 1, pool, st);
 }
@@ -63,6 +66,21 @@ using polfed::fail;
 extern "C" {
 
 const char* polfed_last_error(void) { return polfed::g_error.c_str(); }
+
+int polfed_release_scratch(void) {
+  int dev = 0;
+  POLFED_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= polfed::kMaxDev) return POLFED_OK;
+  cudaMemPool_t pool;
+  {
+    std::lock_guard<std::mutex> lock(polfed::g_pool_mu);
+    pool = polfed::g_pools[dev];
+  }
+  if (!pool) return POLFED_OK;
+  POLFED_CUDA(cudaDeviceSynchronize());
+  POLFED_CUDA(cudaMemPoolTrimTo(pool, 0));
+  return POLFED_OK;
+}
 
 int polfed_version(void) { return 100; }  // 0.1.0
 

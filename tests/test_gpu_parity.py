@@ -294,6 +294,11 @@ def test_filter_host_entry_point_equals_device_entry_point(P):
     got_host = run_filter(P, ham, a, b, coeffs, V, host=True)
     assert np.array_equal(got_dev, got_host)
     assert rel_l2(got_host, core.clenshaw(H, a, b, coeffs, V)) <= 1e-9
+    # the host entry keeps its device blocks in the library's pool; releasing them is harmless
+    free0 = torch.cuda.mem_get_info()[0]
+    P.polfed_release_scratch()
+    assert torch.cuda.mem_get_info()[0] >= free0
+    assert np.array_equal(run_filter(P, ham, a, b, coeffs, V, host=True), got_host)
 
 
 def test_filter_rejects_bad_arguments(P):
