@@ -253,6 +253,21 @@ def test_filter_small_orders_and_edge_cases(P, K, s):
     assert rel_l2(got, want) <= 1e-12
 
 
+@pytest.mark.parametrize("K", [1, 2, 3, 17, 400])
+@pytest.mark.parametrize("n,s", [(8200, 32), (16500, 16)])
+def test_filter_single_launch_path_small_orders(P, K, n, s):
+    """n * s just above the limit of the persistent small-matrix kernels: one fused launch per
+    recurrence step (chained by programmatic dependent launch), first step without b_{k+2}, last
+    step with factor 1, in-place rotation of two buffers."""
+    H = random_csr(n, 6, seed=K + n)
+    V = workloads.start_block(n, s, seed=78)
+    a, b = -0.2, 35.0
+    coeffs = np.random.default_rng(K + 5).standard_normal(K + 1)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    got = run_filter(P, ham_from_oracle(P, H), a, b, coeffs, V)
+    assert rel_l2(got, want) <= 1e-12
+
+
 def bounds_and_coeffs(w, H, K=None):
     v0 = workloads.start_block(H.n, 1, seed=3000 + w.config)[:, 0]
     from oracle import lanczos
