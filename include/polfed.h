@@ -290,6 +290,36 @@ int polfed_block_gram(int s, int64_t n, const double* d_Q, int n_panels, int64_t
 int polfed_block_update(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
                         const double* d_C, double alpha, double beta, double* d_B, void* stream);
 
+/* polfed_block_gram for callers that must not allocate device memory.
+ *
+ * Who needs it: a solver that has given all free HBM to its Krylov basis V_{1:m} (PAPER.md:469, 619:
+ * the basis is the dominant memory), so that one more cudaMalloc -- or growth of the library's
+ * scratch pool, which polfed_block_gram draws from -- fails; a process held to a fixed device-memory
+ * budget by its scheduler or an MPS limit; a latency-bound loop that cannot take the device-wide
+ * synchronisation the CUDA allocator may impose.  This entry point calls no cudaMalloc, cudaFree,
+ * pool or other allocating routine.  Same arguments, same result layout and the same fixed-order
+ * (bit-reproducible) sums as polfed_block_gram; the caller still owns d_Q, d_B and d_C.
+ *
+ * The per-CTA partial sums live in ONE array of POLFED_STATIC_GRAM_DOUBLES doubles (4 MiB) that is
+ * part of the library's device image: every GPU that loads libpolfed.so holds those 4 MiB until the
+ * process exits, whether or not this function is ever called.
+ *   - Limit: n_panels * s * s <= POLFED_STATIC_GRAM_DOUBLES (s = 32: 512 panels; s = 16: 2048), else
+ *     POLFED_ERANGE and nothing is launched.  Split a longer panel list over several calls.  When the
+ *     grid polfed_block_gram would use needs more partial sums than fit, a smaller grid is taken:
+ *     the result then differs from polfed_block_gram's in the last bits (another summation order),
+ *     and is still the same on every run.
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, with
+ *     that device current) and keeps it; make that first call outside any stream capture.
+ *   - All calls share the array and it keeps whatever the last call left.  Nothing in it has to start
+ *     at zero: each call overwrites every slot it later reads.  For the same reason two calls that
+ *     run on the GPU at the same time (different streams, or different host threads on different
+ *     streams) race on it and both results are garbage -- order them on one stream or with events.
+ * Errors: POLFED_EINVAL (s, negative sizes, variant, NULL, d_Q / d_B not 16-byte aligned),
+ * POLFED_ERANGE (the limit above), POLFED_ECUDA (address lookup or launch failed). */
+#define POLFED_STATIC_GRAM_DOUBLES 524288
+int polfed_block_gram_static(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
+                             const double* d_B, double* d_C, int variant, void* stream);
+
 typedef struct {
   double tol;             /* absolute bound on ||H x - lambda x||; <= 0: 1e-8 * max(|E_min|,|E_max|) */
   int32_t max_krylov_dim; /* <= 0: 5 nev + 8 s rounded up to a multiple of s (R10), capped by n and by free memory */

@@ -13,5 +13,5 @@ from .binding import (  # noqa: F401
     polfed_filter_apply_host, polfed_filter_coeffs,
     polfed_spectrum_bounds, polfed_block_lanczos_eigs,
     polfed_kpm_workspace_bytes, polfed_kpm_moments, polfed_kpm_dos,
-    polfed_block_gram, polfed_block_update,
+    polfed_block_gram, polfed_block_update, polfed_block_gram_static, STATIC_GRAM_DOUBLES,
 )

@@ -29,7 +29,7 @@ EXPORTS = (
     "polfed_filter_apply_host", "polfed_filter_coeffs",
     "polfed_spectrum_bounds", "polfed_block_lanczos_eigs",
     "polfed_kpm_workspace_bytes", "polfed_kpm_moments", "polfed_kpm_dos",
-    "polfed_block_gram", "polfed_block_update",
+    "polfed_block_gram", "polfed_block_update", "polfed_block_gram_static",
 )
 
 
@@ -113,6 +113,7 @@ def lib() -> C.CDLL:
     L.polfed_kpm_dos.argtypes = [p, i32, p, i32, p]
     L.polfed_block_gram.argtypes = [i32, i64, p, i32, i64, p, p, i32, p]
     L.polfed_block_update.argtypes = [i32, i64, p, i32, i64, p, f64, f64, p, p]
+    L.polfed_block_gram_static.argtypes = [i32, i64, p, i32, i64, p, p, i32, p]
     _lib = L
     return L
 
@@ -385,6 +386,25 @@ def polfed_block_gram(Q, B, variant: int = 0, stream=None):
     _check(lib().polfed_block_gram(s, n, _dev(Q), k, n * s, _block(B, n, s), _dev(Cm), variant,
                                    _stream(stream)))
     return Cm
+
+
+STATIC_GRAM_DOUBLES = 524288   # POLFED_STATIC_GRAM_DOUBLES of include/polfed.h
+
+
+def polfed_block_gram_static(Q, B, out, variant: int = 0, stream=None):
+    """polfed_block_gram without any device allocation, for callers that cannot allocate (all HBM
+    already given to the Krylov basis, a fixed device-memory budget, or a loop that must not meet the
+    allocator's synchronisation): the partial sums go to a 4 MiB array inside the library.  The
+    wrapper allocates nothing either, so the result tensor `out` (k x s x s, fp64, CUDA) is the
+    caller's.  Needs k*s*s <= STATIC_GRAM_DOUBLES (else PolfedError, code ERANGE).  Calls share
+    the array: never let two of them overlap on the GPU.  Returns `out`."""
+    import torch
+    k, n, s = Q.shape
+    if out.dtype != torch.float64 or tuple(out.shape) != (k, s, s):
+        raise ValueError(f"out must be an fp64 CUDA tensor of shape {(k, s, s)}")
+    _check(lib().polfed_block_gram_static(s, n, _dev(Q), k, n * s, _block(B, n, s), _dev(out),
+                                          variant, _stream(stream)))
+    return out
 
 
 def polfed_block_update(Q, Cm, B, alpha: float, beta: float, stream=None) -> None:

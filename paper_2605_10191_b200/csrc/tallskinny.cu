@@ -9,6 +9,8 @@
 // For s in {8, 16, 32} the Gram product runs on the fp64 tensor cores (mma.sync m8n8k4, operands
 // straight from global memory into fragments); the shared-memory FMA kernel serves s < 8 and is
 // the measured alternative (profiles/r02_reorth.md).
+#include <mutex>
+
 #include "common.cuh"
 
 namespace polfed {
@@ -399,6 +401,65 @@ int resid_launch(long long n, const double* A, const double* B, const double* e,
   return sum_partials((int)grid, S, partial.p, out, st);
 }
 
+// ---- the Gram product for callers that must not allocate (polfed_block_gram_static) ------------
+// The per-CTA partial sums of gram_kernel / gram_dmma_kernel normally sit in a block taken from
+// the library's stream-ordered pool.  Some callers cannot afford that: a solver that has already
+// handed every free byte of HBM to its Krylov basis (any further cudaMalloc or pool growth then
+// fails), a process running under a fixed device-memory budget (an MPS or scheduler limit), or a
+// latency-bound loop that must not hit the implicit device-wide synchronisation of the CUDA
+// allocator.  For them the partial sums go into this fixed array in the library's own device
+// image.  It costs kStaticGramDoubles * 8 bytes = 4 MiB on every GPU that loads libpolfed.so, from
+// load until the process exits.
+//
+// In host code `g_gram_static` is only a handle for the symbol, never a device address (a kernel
+// given `g_gram_static` from the host would fault, or quietly use host memory where the GPU can
+// reach it); static_gram_scratch() asks the runtime for the real address once per device, with
+// that device current, and the launches below get that pointer.
+constexpr size_t kStaticGramDoubles = POLFED_STATIC_GRAM_DOUBLES;
+static __device__ __align__(256) double g_gram_static[kStaticGramDoubles];
+
+std::mutex g_static_mu;
+double* g_static_ptr[64] = {};  // by device ordinal; filled on the first call on that device
+
+int static_gram_scratch(double** out) {
+  int dev = 0;
+  POLFED_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(POLFED_EINVAL, "polfed_block_gram_static: device ordinal %d", dev);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ptr[dev]) {
+    double* ptr = nullptr;
+    POLFED_CUDA(cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_gram_static));
+    if (!ptr) return fail(POLFED_ECUDA, "polfed_block_gram_static: no device address for the static scratch");
+    g_static_ptr[dev] = ptr;
+  }
+  *out = g_static_ptr[dev];
+  return POLFED_OK;
+}
+
+// gram_launch with the partial sums in `scratch` (kStaticGramDoubles doubles).  The grid is the one
+// gram_launch would take, cut down until gx * n_panels * S * S partial sums fit; every slot that
+// sum_partials reads is written by this call's own CTAs first (a CTA without rows writes zeros),
+// so what an earlier call left in the array is never read and nothing has to be cleared.
+template <int S>
+int gram_launch_static(long long n, const double* Q, int n_panels, size_t stride, const double* B, double* C,
+                       int sm_count, int variant, double* scratch, cudaStream_t st) {
+  const size_t len = (size_t)n_panels * S * S;
+  const bool use_dmma = S >= 8 && variant != 1;
+  const long long work = use_dmma ? (n / 4 + kDmmaThreads / 32 - 1) / (kDmmaThreads / 32)
+                                  : (n + kTileRows - 1) / kTileRows;
+  long long gx = (long long)sm_count * 8 / n_panels;
+  if (gx > work) gx = work;
+  if (gx > (long long)(kStaticGramDoubles / len)) gx = (long long)(kStaticGramDoubles / len);
+  if (gx < 1) gx = 1;
+  dim3 grid((unsigned)gx, (unsigned)n_panels);
+  if constexpr (S >= 8) {
+    if (use_dmma) gram_dmma_kernel<S><<<grid, kDmmaThreads, 0, st>>>(n, Q, stride, B, scratch);
+  }
+  if (!use_dmma) gram_kernel<S><<<grid, kTsThreads, 0, st>>>(n, Q, stride, B, scratch);
+  POLFED_LAUNCH_CHECK("gram_kernel (static scratch)");
+  return sum_partials((int)gx, len, scratch, C, st);
+}
+
 }  // namespace
 
 #define POLFED_BY_S(s, CALL)                                                     \
@@ -426,7 +487,10 @@ int ts_gram_variant(int s, long long n, const double* Q, int n_panels, size_t st
   POLFED_BY_S(s, (gram_launch<S_>(n, Q, n_panels, stride, B, d_C, sm_count, variant, st)));
 }
 
-
+int ts_gram_static(int s, long long n, const double* Q, int n_panels, size_t stride, const double* B,
+                   double* d_C, int sm_count, int variant, double* scratch, cudaStream_t st) {
+  POLFED_BY_S(s, (gram_launch_static<S_>(n, Q, n_panels, stride, B, d_C, sm_count, variant, scratch, st)));
+}
 
 int ts_update(int s, long long n, const double* Q, int n_panels, size_t stride, const double* d_C,
               double alpha, double beta, double* B, cudaStream_t st) {
@@ -482,6 +546,29 @@ int polfed_block_gram(int s, int64_t n, const double* d_Q, int n_panels, int64_t
   if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   return polfed::ts_gram_variant(s, n, d_Q, n_panels, (size_t)panel_stride, d_B, d_C, sms, variant,
                                  static_cast<cudaStream_t>(stream));
+}
+
+int polfed_block_gram_static(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
+                             const double* d_B, double* d_C, int variant, void* stream) {
+  if (!polfed::valid_block_size(s))
+    return fail(POLFED_EINVAL, "polfed_block_gram_static: bad block size s=%d", s);
+  if (n < 0 || n_panels < 0 || panel_stride < 0 || variant < 0 || variant > 2)
+    return fail(POLFED_EINVAL, "polfed_block_gram_static: bad argument");
+  if (n == 0 || n_panels == 0) return POLFED_OK;
+  if ((long long)n_panels * s * s > (long long)POLFED_STATIC_GRAM_DOUBLES)
+    return fail(POLFED_ERANGE,
+                "polfed_block_gram_static: n_panels*s*s = %lld partial sums per CTA row exceed the static "
+                "scratch of %d doubles (POLFED_STATIC_GRAM_DOUBLES); split the panels over several calls "
+                "or use polfed_block_gram",
+                (long long)n_panels * s * s, (int)POLFED_STATIC_GRAM_DOUBLES);
+  if (!d_Q || !d_B || !d_C || !polfed::aligned16(d_Q) || !polfed::aligned16(d_B))
+    return fail(POLFED_EINVAL, "polfed_block_gram_static: NULL or misaligned block");
+  double* scratch = nullptr;
+  if (int rc = polfed::static_gram_scratch(&scratch)) return rc;
+  int dev = 0, sms = 148;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  return polfed::ts_gram_static(s, n, d_Q, n_panels, (size_t)panel_stride, d_B, d_C, sms, variant, scratch,
+                                static_cast<cudaStream_t>(stream));
 }
 
 int polfed_block_update(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
