@@ -40,7 +40,9 @@ enum {
   POLFED_ECUDA = 3,      /* a CUDA call or kernel launch failed */
   POLFED_ERANGE = 4,     /* rescaled target outside (-1,1), b <= 0, index overflow */
   POLFED_ENOCONV = 5,    /* eigen-solver hit max_krylov_dim before nev pairs converged */
-  POLFED_EBREAKDOWN = 6  /* rank-deficient Krylov block (R17) */
+  POLFED_EBREAKDOWN = 6, /* rank-deficient Krylov block (R17) */
+  POLFED_EWINDOW = 7     /* eigen-solver: every extracted pair converged, but the filter's main lobe
+                            holds fewer than nev levels (order K too high); outputs are valid eigenpairs */
 };
 
 typedef struct polfed_basis polfed_basis;
@@ -161,9 +163,26 @@ int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_term* h_ter
  * at most 3 bits, off-diagonal terms of kind XX only, at most 64 of them outside bits 0-2. */
 
 /* Wrap a caller-owned device CSR (any real symmetric matrix, columns < n, row_ptr[n] == nnz).
- * The arrays are NOT copied and must outlive the handle. */
+ * The three arrays are kept by pointer and must outlive the handle.  They must be COMPLETE when the
+ * call is made: it launches kernels that read them (the longest row for n <= 262144; a scan of the
+ * values) and synchronises before returning.  polfed_ham_from_csr runs that work on the legacy
+ * default stream; use polfed_ham_from_csr_ex to give the stream the arrays were produced on.
+ *
+ * The VALUES ARE SNAPSHOTTED when the off-diagonal entries take one or two distinct values (every
+ * XXZ chain): the handle then also holds a packed copy (dense diagonal + 4-byte column words,
+ * 4 B per entry + 12 n bytes of device memory) and the fused-step kernel reads that copy, not
+ * d_val (the persistent small-matrix filter still reads d_val).  A caller that later changes d_val
+ * in place must either build a new handle or pass POLFED_HAM_NO_SNAPSHOT: the handle then holds no
+ * copy of any value, skips that pass over the entries, and every step reads d_val as it is at that
+ * moment (plain CSR kernel: 12 instead of 4 bytes per stored entry; XXZ L = 20, s = 16 in round 1:
+ * 32.7 against 26.6 us per step).  The structure (row_ptr, col) must never change under a handle.
+ * Errors: POLFED_EINVAL (NULL, negative size, d_val not 16-byte / d_col not 4-byte aligned, unknown
+ * flag), POLFED_ERANGE (n or nnz >= 2^31), POLFED_ENOMEM, POLFED_ECUDA. */
+enum { POLFED_HAM_NO_SNAPSHOT = 1 };
 int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const int32_t* d_col,
                         const double* d_val, polfed_ham** out);
+int polfed_ham_from_csr_ex(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const int32_t* d_col,
+                           const double* d_val, unsigned flags, void* stream, polfed_ham** out);
 int polfed_ham_destroy(polfed_ham* ham);
 /* Any output pointer may be NULL. */
 int polfed_ham_csr(const polfed_ham* ham, int64_t* n, int64_t* nnz, const int32_t** d_row_ptr,
@@ -248,7 +267,13 @@ int polfed_filter_coeffs(double a, double b, double sigma, int nev, double rho_r
  * *a = (hi+lo)/2, *b = (1+margin)(hi-lo)/2 (Eq. 31 widened by `margin`, R5; margin < 0
  * means the default 0.01).  Ritz values lie inside the spectrum, so a and b are computed from
  * the extremal Ritz values moved outwards by their residual norms beta_{m+1} |z_m| (Eq. 6, 16;
- * zero once they have converged); *emin, *emax are the Ritz values themselves.
+ * zero once they have converged); *emin, *emax are the Ritz values themselves.  This is a
+ * HEURISTIC, not an enclosure: the residual only guarantees SOME eigenvalue within that distance of
+ * the Ritz value, not that E_max <= theta_max + residual.  With too few steps on a spectrum with
+ * thin tails the true extremes can lie outside [a - b, a + b]; polfed_filter_apply then grows like
+ * cosh(K acosh|x|) on those levels.  polfed_block_lanczos_eigs detects that (POLFED_ERANGE);
+ * callers of polfed_filter_apply who need a guarantee should pass an enclosure of their own (e.g.
+ * a Gershgorin bound) as a, b.
  * n_steps <= 0 means 60 (R6); it is clipped to n.  Allocates
  * (n_steps+1) x n doubles of device scratch and frees it; synchronises `stream`. */
 int polfed_spectrum_bounds(const polfed_ham* ham, int n_steps, const double* d_v0, double margin,
@@ -280,7 +305,8 @@ int polfed_kpm_dos(const double* h_moments, int n_moments, const double* e_resca
  *   polfed_block_gram:    C_j = Q_j^T B      for j < n_panels   (C: n_panels x s x s, row-major)
  *   polfed_block_update:  B = beta B + alpha sum_j Q_j C_j
  * Q_j = d_Q + j * panel_stride doubles, each n x s row-major like B; s in {1,2,4,8,16,32}; all
- * pointers DEVICE, 16-byte aligned.  Every sum runs in a fixed order (bit-reproducible).
+ * pointers DEVICE, 16-byte aligned, panel_stride >= n*s when there is more than one panel (else
+ * POLFED_EINVAL, nothing is launched).  Every sum runs in a fixed order (bit-reproducible).
  * variant: 0 = the library's choice (fp64 tensor-core mma for s >= 8), 1 = the shared-memory FMA
  * kernel, 2 = tensor cores (s >= 8 only, else the FMA kernel).  Enqueued on `stream`; scratch for
  * the per-CTA partial sums comes from the library's stream-ordered pool (see
@@ -314,8 +340,8 @@ int polfed_block_update(int s, int64_t n, const double* d_Q, int n_panels, int64
  *     at zero: each call overwrites every slot it later reads.  For the same reason two calls that
  *     run on the GPU at the same time (different streams, or different host threads on different
  *     streams) race on it and both results are garbage -- order them on one stream or with events.
- * Errors: POLFED_EINVAL (s, negative sizes, variant, NULL, d_Q / d_B not 16-byte aligned),
- * POLFED_ERANGE (the limit above), POLFED_ECUDA (address lookup or launch failed). */
+ * Errors: POLFED_EINVAL (s, negative sizes, variant, NULL, a pointer not 16-byte aligned, overlapping
+ * panels), POLFED_ERANGE (the limit above), POLFED_ECUDA (address lookup or launch failed). */
 #define POLFED_STATIC_GRAM_DOUBLES 524288
 int polfed_block_gram_static(int s, int64_t n, const double* d_Q, int n_panels, int64_t panel_stride,
                              const double* d_B, double* d_C, int variant, void* stream);
@@ -379,7 +405,14 @@ typedef struct {
  * d_V0: n x s start block (need not be orthonormal; full column rank required).
  * Outputs: h_evals[nev] ascending, d_evecs n x nev row-major (column j pairs with h_evals[j]),
  * h_residuals[nev]; report may be NULL.  Returns POLFED_ENOCONV (outputs hold the best nev
- * pairs found) if max_krylov_dim is reached first, POLFED_EBREAKDOWN on a rank-deficient block.
+ * pairs found) if max_krylov_dim is reached first, POLFED_EBREAKDOWN on a rank-deficient block,
+ * POLFED_EWINDOW as soon as all nev + s (rounded up) extracted pairs are converged while fewer than
+ * nev of them lie in the main lobe (the density of states was overestimated, so K is too high and
+ * the window too narrow: the outputs are the nev converged eigenpairs nearest sigma, possibly not
+ * contiguous; call again with a lower K_override or a larger window_levels), and POLFED_ERANGE when
+ * a Rayleigh-Ritz value of H falls outside [a - b, a + b]: the bounds of step 1 are extremal Ritz
+ * values moved outwards by their residuals and a margin -- a heuristic, NOT an enclosure (R5) -- and
+ * a spectrum that sticks out makes the filter grow without bound there.
  * Allocates the Krylov basis (max_krylov_dim + s columns) and scratch on the device;
  * synchronises `stream`. */
 int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int s, const double* d_V0,

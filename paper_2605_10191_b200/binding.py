@@ -15,15 +15,17 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpolfed.so")
 
-OK, EINVAL, ENOMEM, ECUDA, ERANGE, ENOCONV, EBREAKDOWN = range(7)
+OK, EINVAL, ENOMEM, ECUDA, ERANGE, ENOCONV, EBREAKDOWN, EWINDOW = range(8)
 TERM_KINDS = {"ZZ": 0, "Z": 1, "NN": 2, "N": 3, "EXCH": 4, "HOPJW": 5, "XX": 6}
 FORMAT_CSR, FORMAT_TILED, FORMAT_FLIP, FORMAT_SECTOR = 0, 2, 3, 4
+HAM_NO_SNAPSHOT = 1
 
 EXPORTS = (
     "polfed_last_error", "polfed_version", "polfed_release_scratch",
     "polfed_build_basis", "polfed_basis_destroy", "polfed_basis_dim", "polfed_basis_states",
     "polfed_basis_rank",
-    "polfed_build_hamiltonian", "polfed_ham_from_csr", "polfed_ham_destroy", "polfed_ham_csr",
+    "polfed_build_hamiltonian", "polfed_ham_from_csr", "polfed_ham_from_csr_ex", "polfed_ham_destroy",
+    "polfed_ham_csr",
     "polfed_fused_step", "polfed_filter_workspace_bytes", "polfed_filter_workspace_bytes_ham",
     "polfed_filter_apply",
     "polfed_filter_apply_host", "polfed_filter_coeffs",
@@ -92,6 +94,7 @@ def lib() -> C.CDLL:
     L.polfed_basis_rank.argtypes = [p, p, i64, p, p]
     L.polfed_build_hamiltonian.argtypes = [p, p, i32, p, i32, p, C.POINTER(p)]
     L.polfed_ham_from_csr.argtypes = [i64, i64, p, p, p, C.POINTER(p)]
+    L.polfed_ham_from_csr_ex.argtypes = [i64, i64, p, p, p, C.c_uint, p, C.POINTER(p)]
     L.polfed_ham_destroy.argtypes = [p]
     L.polfed_ham_csr.argtypes = [p, C.POINTER(i64), C.POINTER(i64), C.POINTER(p), C.POINTER(p),
                                  C.POINTER(p)]
@@ -271,6 +274,19 @@ def polfed_ham_from_csr(row_ptr, col, val) -> Ham:
     n, nnz = row_ptr.numel() - 1, col.numel()
     h = C.c_void_p()
     _check(lib().polfed_ham_from_csr(n, nnz, _dev(row_ptr), _dev(col), _dev(val), C.byref(h)))
+    return Ham(h.value, keep=(row_ptr, col, val))
+
+
+def polfed_ham_from_csr_ex(row_ptr, col, val, flags: int = 0, stream=None) -> Ham:
+    """polfed_ham_from_csr with flags (HAM_NO_SNAPSHOT: the handle keeps no copy of the values, so
+    in-place updates of `val` are seen by later steps) and the stream the arrays were written on."""
+    import torch
+    if row_ptr.dtype != torch.int32 or col.dtype != torch.int32 or val.dtype != torch.float64:
+        raise ValueError("CSR tensors must be int32, int32, float64")
+    n, nnz = row_ptr.numel() - 1, col.numel()
+    h = C.c_void_p()
+    _check(lib().polfed_ham_from_csr_ex(n, nnz, _dev(row_ptr), _dev(col), _dev(val), flags,
+                                        _stream(stream), C.byref(h)))
     return Ham(h.value, keep=(row_ptr, col, val))
 
 
@@ -454,7 +470,8 @@ def polfed_block_lanczos_eigs(ham: Ham, sigma: float, nev: int, s: int, V0, *, t
                               allow_unconverged: bool = False, kpm_block=None,
                               kpm_moments: int = 0, window_levels: int = 0):
     """The nev eigenpairs of H nearest sigma: (evals ndarray, evecs CUDA tensor n x nev,
-    residuals ndarray, report dict).  Raises PolfedError(ENOCONV) unless allow_unconverged.
+    residuals ndarray, report dict).  Raises PolfedError(ENOCONV or EWINDOW) unless allow_unconverged
+    (report["status"] then holds the code).
     kpm_block (CUDA tensor n x R, R a multiple of 4): size K with the KPM density of states.
     window_levels > 0: size the filter window for that many levels instead of nev + 10 %."""
     import torch
@@ -474,7 +491,7 @@ def polfed_block_lanczos_eigs(ham: Ham, sigma: float, nev: int, s: int, V0, *, t
                                            _block(V0, ham.n, s), C.byref(opt), evals.ctypes.data,
                                            _dev(evecs), resid.ctypes.data, C.byref(rep),
                                            _stream(stream))
-    if not (code == ENOCONV and allow_unconverged):
+    if not (code in (ENOCONV, EWINDOW) and allow_unconverged):
         _check(code)
     report = {name: getattr(rep, name) for name, _ in _Report._fields_ if name != "reserved"}
     report["status"] = code

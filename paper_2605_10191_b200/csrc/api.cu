@@ -84,17 +84,20 @@ int polfed_release_scratch(void) {
 
 int polfed_version(void) { return 100; }  // 0.1.0
 
-int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const int32_t* d_col,
-                        const double* d_val, polfed_ham** out) {
+int polfed_ham_from_csr_ex(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const int32_t* d_col,
+                           const double* d_val, unsigned flags, void* stream, polfed_ham** out) {
   if (!out) return fail(POLFED_EINVAL, "polfed_ham_from_csr: out is NULL");
   *out = nullptr;
   if (n < 0 || nnz < 0) return fail(POLFED_EINVAL, "polfed_ham_from_csr: negative size");
+  if (flags & ~(unsigned)POLFED_HAM_NO_SNAPSHOT)
+    return fail(POLFED_EINVAL, "polfed_ham_from_csr_ex: unknown flag bits 0x%x", flags);
   if (n >= (int64_t(1) << 31) || nnz >= (int64_t(1) << 31))
     return fail(POLFED_ERANGE, "polfed_ham_from_csr: n and nnz must fit int32 indices");
   if (!d_row_ptr || (nnz > 0 && (!d_col || !d_val)))
     return fail(POLFED_EINVAL, "polfed_ham_from_csr: NULL array");
   if (!polfed::aligned16(d_val) || (reinterpret_cast<uintptr_t>(d_col) & 3u))
     return fail(POLFED_EINVAL, "polfed_ham_from_csr: misaligned array");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
   polfed_ham* h = new (std::nothrow) polfed_ham;
   if (!h) return fail(POLFED_ENOMEM, "polfed_ham_from_csr: host allocation failed");
   h->n = n;
@@ -109,14 +112,15 @@ int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const 
   h->sm_count = sms > 0 ? sms : 148;
   cudaGetLastError();
   if (n <= 262144) {  // only the persistent small-matrix filter asks for it
-    int rc = polfed::csr_max_row_len(n, d_row_ptr, &h->max_row_len);
+    int rc = polfed::csr_max_row_len(n, d_row_ptr, &h->max_row_len, st);
     if (rc) {
       delete h;
       return rc;
     }
   }
-  {  // the packed form of the same matrix, when its off-diagonal values are few (packed.cuh)
-    int rc = polfed::build_packed_plan(h, nullptr, &h->packed);
+  if (!(flags & POLFED_HAM_NO_SNAPSHOT)) {
+    // the packed form of the same matrix, when its off-diagonal values are few (packed.cuh)
+    int rc = polfed::build_packed_plan(h, st, &h->packed);
     if (rc) {
       delete h;
       return rc;
@@ -124,6 +128,11 @@ int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const 
   }
   *out = h;
   return POLFED_OK;
+}
+
+int polfed_ham_from_csr(int64_t n, int64_t nnz, const int32_t* d_row_ptr, const int32_t* d_col,
+                        const double* d_val, polfed_ham** out) {
+  return polfed_ham_from_csr_ex(n, nnz, d_row_ptr, d_col, d_val, 0u, nullptr, out);
 }
 
 int polfed_ham_destroy(polfed_ham* ham) {

@@ -311,7 +311,10 @@ extern "C" int polfed_build_hamiltonian(const polfed_basis* basis, const polfed_
                         &d_col, &d_val, &total);
   if (rc) return rc;
   polfed_ham* h = nullptr;
-  rc = polfed_ham_from_csr(basis->dim, total, d_row_ptr, d_col, d_val, &h);
+  // the tiled, sector and flip plans carry their own copy of the matrix: their handles keep the
+  // CSR for the steps those plans do not take (s below the plan's sizes) and skip the packed copy
+  rc = polfed_ham_from_csr_ex(basis->dim, total, d_row_ptr, d_col, d_val,
+                              format == POLFED_FORMAT_CSR ? 0u : (unsigned)POLFED_HAM_NO_SNAPSHOT, stream, &h);
   if (rc) {
     cudaFree(d_row_ptr); cudaFree(d_col); cudaFree(d_val);
     return rc;

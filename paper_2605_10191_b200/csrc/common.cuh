@@ -77,7 +77,7 @@ int flip_step(const polfed_ham* ham, int s, double p, double q, double r, double
 // small_filter.cu: the whole recurrence in one persistent kernel (n * s <= 262144).
 // small_filter_apply returns POLFED_ERANGE when it cannot take the matrix (caller: single launches).
 bool small_filter_supports(const polfed_ham* ham, int s);
-int csr_max_row_len(long long n, const int32_t* d_row_ptr, int* out);
+int csr_max_row_len(long long n, const int32_t* d_row_ptr, int* out, cudaStream_t st);
 int small_filter_apply(const polfed_ham* ham, double a, double b, int K, const double* h_coeffs,
                        int s, const double* d_V, double* d_W, double* cur, double* old,
                        cudaStream_t st);

@@ -121,7 +121,10 @@ struct DenseEigh {
 };
 
 // P(x) = sum_k c_k T_k(x) by the scalar Clenshaw recurrence (Eq. 50-51 with H~ -> x).
+// Outside [-1, 1] the series is not the filter any more (it grows without bound): 0 there, so that an
+// out-of-interval level never passes a main-lobe test.
 double filter_value(const std::vector<double>& c, double x) {
+  if (!(std::fabs(x) <= 1.0)) return 0.0;
   double b1 = 0.0, b2 = 0.0;
   for (size_t k = c.size() - 1; k >= 1; --k) {
     const double t = c[k] + 2.0 * x * b1 - b2;
@@ -564,6 +567,17 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
     }
     for (int c = 0; c < wp; ++c) res[c] = std::sqrt(std::max(res[c], 0.0));
     rep.seconds_extraction += now_seconds() - t0 - t_eig_inside;
+    // The bounds of step 1 are a heuristic, not an enclosure (R5).  A Rayleigh-Ritz value of H
+    // itself never leaves [E_min, E_max], so one outside [a - b, a + b] proves that the spectrum
+    // sticks out of the Chebyshev interval: there P grows like cosh(K acosh|x|) and swamps the window.
+    for (int c = 0; c < wp; ++c) {
+      const double x = (Eg[c] - a_) / b_;
+      if (std::fabs(x) > 1.0)
+        return fail(POLFED_ERANGE,
+                    "polfed_block_lanczos_eigs: Ritz value %.17g of H lies outside [a - b, a + b] = [%.17g, %.17g] "
+                    "(rescaled %.6f): the spectral bounds are too tight; raise bounds_steps or bounds_margin, "
+                    "or pass a, b", Eg[c], a_ - b_, a_ + b_, x);
+    }
 
     // -- selection (R11): converged pairs nearest sigma
     std::vector<int> order(wp);
@@ -585,13 +599,18 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
     rep.n_converged = std::min(n_lead, nev);
     std::vector<int> sel;
     const bool done = n_lead >= nev;
-    if (done) {
+    // Every extracted pair converged, yet fewer than nev of them in the main lobe: the wp levels
+    // with the largest P are all known, so the lobe holds fewer than nev levels (density of states
+    // overestimated, K too high) and no further block step can change that.  Stop here instead of
+    // running to max_krylov_dim; the outputs are the nev converged pairs nearest sigma.
+    const bool narrow = !done && (int)good.size() == wp;
+    if (done || narrow) {
       sel.assign(good.begin(), good.begin() + nev);
     } else {
       sel.assign(order.begin(), order.begin() + nev);
     }
     std::sort(sel.begin(), sel.end(), [&](int x, int y) { return Eg[x] < Eg[y]; });
-    if (done || k == k_cap || !have_best) {
+    if (done || narrow || k == k_cap || !have_best) {
       // write the outputs (best effort until converged)
       for (int j = 0; j < nev; ++j) {
         h_evals[j] = Eg[sel[j]];
@@ -613,6 +632,10 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
       status = POLFED_OK;
       break;
     }
+    if (narrow) {
+      status = POLFED_EWINDOW;
+      break;
+    }
     const int missing = nev - std::min(n_lead, nev);
     next_check = opt.check_every > 0 ? k + opt.check_every : k + std::max(1, (missing + 2 * s - 1) / (2 * s));
   }
@@ -627,6 +650,12 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
   rep.K = K;
   rep.seconds_total = now_seconds() - t_start;
   if (report) *report = rep;
+  if (status == POLFED_EWINDOW)
+    return fail(POLFED_EWINDOW,
+                "polfed_block_lanczos_eigs: all %d extracted pairs are converged eigenpairs but only %d lie in the "
+                "main lobe of the filter (K = %d is too high for nev = %d: density of states overestimated); "
+                "the outputs hold the nev converged pairs nearest sigma; lower K_override or raise window_levels",
+                wp, rep.n_converged, K, nev);
   if (status == POLFED_ENOCONV)
     return fail(POLFED_ENOCONV, "polfed_block_lanczos_eigs: %d of %d pairs converged at Krylov dimension %d",
                 rep.n_converged, nev, rep.krylov_dim);

@@ -11,6 +11,7 @@
 #include <cooperative_groups.h>
 
 #include <algorithm>
+#include <mutex>
 
 #include "common.cuh"
 
@@ -269,15 +270,19 @@ bool small_filter_supports(const polfed_ham* ham, int s) {
   return ham->n * (long long)s <= kGridItems;
 }
 
-// Longest row of a CSR matrix (polfed_ham_from_csr records it in the handle).  Synchronises.
-int csr_max_row_len(long long n, const int32_t* d_row_ptr, int* out) {
+// Longest row of a CSR matrix (polfed_ham_from_csr records it in the handle).  Runs on `st` and
+// synchronises it.
+int csr_max_row_len(long long n, const int32_t* d_row_ptr, int* out, cudaStream_t st) {
   *out = 0;
   if (n < 1) return POLFED_OK;
   int* d_max = nullptr;
   POLFED_CUDA(cudaMalloc(&d_max, sizeof(int)));
-  cudaMemset(d_max, 0, sizeof(int));
-  max_row_len_kernel<<<(unsigned)((n + 255) / 256), 256>>>(n, d_row_ptr, d_max);
-  cudaError_t e = cudaMemcpy(out, d_max, sizeof(int), cudaMemcpyDeviceToHost);
+  cudaError_t e = cudaMemsetAsync(d_max, 0, sizeof(int), st);
+  if (e == cudaSuccess) {
+    max_row_len_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, d_row_ptr, d_max);
+    e = cudaMemcpyAsync(out, d_max, sizeof(int), cudaMemcpyDeviceToHost, st);
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   cudaFree(d_max);
   if (e != cudaSuccess) return fail(POLFED_ECUDA, "csr_max_row_len: %s", cudaGetErrorString(e));
   return POLFED_OK;
@@ -287,14 +292,25 @@ int csr_max_row_len(long long n, const int32_t* d_row_ptr, int* out) {
 int small_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const double* c, int s,
                        const double* d_V, double* d_W, double* cur, double* old, cudaStream_t st) {
   constexpr int kSmemCap = 200 * 1024;
-  static int coop = -1;
-  if (coop < 0) {
-    int dev = 0;
-    POLFED_CUDA(cudaGetDevice(&dev));
-    POLFED_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
-    for (int v = 0; v < 8; ++v)
-      POLFED_CUDA(cudaFuncSetAttribute(kKernels[v], cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       kSmemCap));
+  // The shared-memory opt-in of a kernel and the cooperative-launch capability belong to a device,
+  // not to the process: set / query them once per device ordinal (any thread may get here first).
+  constexpr int kMaxDev = 64;
+  static std::mutex mu;
+  static int coop_of[kMaxDev];
+  static bool ready[kMaxDev] = {};
+  int dev = 0, coop = 0;
+  POLFED_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDev) return POLFED_ERANGE;  // caller: single launches
+  {
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ready[dev]) {
+      POLFED_CUDA(cudaDeviceGetAttribute(&coop_of[dev], cudaDevAttrCooperativeLaunch, dev));
+      for (int v = 0; v < 8; ++v)
+        POLFED_CUDA(cudaFuncSetAttribute(kKernels[v], cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         kSmemCap));
+      ready[dev] = true;
+    }
+    coop = coop_of[dev];
   }
   const int items = (int)ham->n * s;
   const bool single = items <= kSingleItems;
@@ -338,9 +354,18 @@ int small_filter_apply(const polfed_ham* ham, double a_, double b_, int K, const
                                    2 * (size_t)items * sizeof(double), st));
     else if (single)
       POLFED_CUDA(cudaLaunchKernel(kernel, dim3(1), dim3(kSingleThreads), params, smem, st));
-    else
-      POLFED_CUDA(cudaLaunchCooperativeKernel(kernel, dim3((unsigned)grid), dim3((unsigned)threads),
-                                              params, smem, st));
+    else {
+      const cudaError_t le = cudaLaunchCooperativeKernel(kernel, dim3((unsigned)grid),
+                                                         dim3((unsigned)threads), params, smem, st);
+      // a device (or an MPS / green-context share of one) that cannot hold the whole grid at once:
+      // nothing has run yet on the first chunk, so the caller can still take the single launches
+      if (k == K - 1 && (le == cudaErrorCooperativeLaunchTooLarge || le == cudaErrorInvalidValue ||
+                         le == cudaErrorLaunchOutOfResources)) {
+        (void)cudaGetLastError();
+        return POLFED_ERANGE;
+      }
+      POLFED_CUDA(le);
+    }
     if (n_steps & 1) std::swap(cur, old);  // the kernel's rotation, seen from the host
     k -= n_steps;
   }

@@ -540,8 +540,11 @@ int polfed_block_gram(int s, int64_t n, const double* d_Q, int n_panels, int64_t
   if (n < 0 || n_panels < 0 || panel_stride < 0 || variant < 0 || variant > 2)
     return fail(POLFED_EINVAL, "polfed_block_gram: bad argument");
   if (n == 0 || n_panels == 0) return POLFED_OK;
-  if (!d_Q || !d_B || !d_C || !polfed::aligned16(d_Q) || !polfed::aligned16(d_B))
+  if (!d_Q || !d_B || !d_C || !polfed::aligned16(d_Q) || !polfed::aligned16(d_B) || !polfed::aligned16(d_C))
     return fail(POLFED_EINVAL, "polfed_block_gram: NULL or misaligned block");
+  if (n_panels > 1 && panel_stride < n * s)
+    return fail(POLFED_EINVAL, "polfed_block_gram: panel_stride %lld < n*s, the panels overlap",
+                (long long)panel_stride);
   int dev = 0, sms = 148;
   if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   return polfed::ts_gram_variant(s, n, d_Q, n_panels, (size_t)panel_stride, d_B, d_C, sms, variant,
@@ -561,8 +564,11 @@ int polfed_block_gram_static(int s, int64_t n, const double* d_Q, int n_panels, 
                 "scratch of %d doubles (POLFED_STATIC_GRAM_DOUBLES); split the panels over several calls "
                 "or use polfed_block_gram",
                 (long long)n_panels * s * s, (int)POLFED_STATIC_GRAM_DOUBLES);
-  if (!d_Q || !d_B || !d_C || !polfed::aligned16(d_Q) || !polfed::aligned16(d_B))
+  if (!d_Q || !d_B || !d_C || !polfed::aligned16(d_Q) || !polfed::aligned16(d_B) || !polfed::aligned16(d_C))
     return fail(POLFED_EINVAL, "polfed_block_gram_static: NULL or misaligned block");
+  if (n_panels > 1 && panel_stride < n * s)
+    return fail(POLFED_EINVAL, "polfed_block_gram_static: panel_stride %lld < n*s, the panels overlap",
+                (long long)panel_stride);
   double* scratch = nullptr;
   if (int rc = polfed::static_gram_scratch(&scratch)) return rc;
   int dev = 0, sms = 148;
@@ -578,6 +584,12 @@ int polfed_block_update(int s, int64_t n, const double* d_Q, int n_panels, int64
   if (n == 0) return POLFED_OK;
   if (!d_B || (n_panels > 0 && (!d_Q || !d_C)))
     return fail(POLFED_EINVAL, "polfed_block_update: NULL block");
+  // the tensor-core kernel moves B in 16-byte pieces: a misaligned B would fault on the device
+  if (!polfed::aligned16(d_B) || (n_panels > 0 && (!polfed::aligned16(d_Q) || !polfed::aligned16(d_C))))
+    return fail(POLFED_EINVAL, "polfed_block_update: blocks must be 16-byte aligned");
+  if (n_panels > 1 && panel_stride < n * s)
+    return fail(POLFED_EINVAL, "polfed_block_update: panel_stride %lld < n*s, the panels overlap",
+                (long long)panel_stride);
   return polfed::ts_update(s, n, d_Q, n_panels, (size_t)panel_stride, d_C, alpha, beta, d_B,
                            static_cast<cudaStream_t>(stream));
 }

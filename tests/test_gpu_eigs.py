@@ -138,6 +138,45 @@ def test_eigs_wider_window_gives_lower_order_and_the_same_pairs(P):
     assert err.value.code == P.binding.EINVAL
 
 
+def test_eigs_window_too_narrow_is_reported_early_with_valid_pairs(P):
+    """with an order K far above what Eq. (40)-(42) give for nev (as after an overestimated
+    density of states) the main lobe holds fewer than nev levels.  Once every extracted pair is a
+    converged eigenpair nothing can change that: the solver must say so (POLFED_EWINDOW) instead of
+    running to max_krylov_dim, and what it returns must be true eigenpairs (dense truth)."""
+    w = workloads.make_workload(1)
+    _, H = core.hamiltonian(w)
+    ev = np.linalg.eigvalsh(H.to_dense())
+    hnorm = max(abs(ev[0]), abs(ev[-1]))
+    V0 = dev(workloads.start_block(H.n, 1, seed=2001, orthonormal=True))
+    ham = build(P, w)
+    _, _, _, rep0 = P.polfed_block_lanczos_eigs(ham, w.target, w.nev, 1, V0, max_krylov_dim=900)
+    K_high = 5 * rep0["K"]
+    with pytest.raises(P.PolfedError) as err:
+        P.polfed_block_lanczos_eigs(ham, w.target, w.nev, 1, V0, K_override=K_high, max_krylov_dim=900)
+    assert err.value.code == P.binding.EWINDOW
+    evals, evecs, resid, rep = P.polfed_block_lanczos_eigs(ham, w.target, w.nev, 1, V0, K_override=K_high,
+                                                           max_krylov_dim=900, allow_unconverged=True)
+    assert rep["status"] == P.binding.EWINDOW and rep["n_converged"] < w.nev
+    assert rep["krylov_dim"] < 900                       # stopped early, not at the cap
+    check_pairs(H, evals, evecs, resid, 1e-8 * hnorm)
+    for lam_ in evals:
+        assert np.min(np.abs(ev - lam_)) <= 1e-9 * hnorm
+
+
+def test_eigs_refuses_an_interval_the_spectrum_sticks_out_of(P):
+    """a, b that do not enclose the spectrum (here: 60 % of its half-width) must come
+    back as POLFED_ERANGE -- a Rayleigh-Ritz value of H outside [a - b, a + b] proves it -- and not as
+    slow or wrong convergence."""
+    w = workloads.make_workload(1)
+    ham = build(P, w)
+    V0 = dev(workloads.start_block(ham.n, 1, seed=2001, orthonormal=True))
+    _, _, _, rep0 = P.polfed_block_lanczos_eigs(ham, w.target, w.nev, 1, V0, max_krylov_dim=900)
+    with pytest.raises(P.PolfedError) as err:
+        P.polfed_block_lanczos_eigs(ham, w.target, w.nev, 1, V0, a=rep0["a"], b=0.6 * rep0["b"],
+                                    K_override=40, max_krylov_dim=900)
+    assert err.value.code == P.binding.ERANGE
+
+
 def test_eigs_reports_no_convergence_and_bad_arguments(P):
     w = workloads.make_workload(1)
     ham = build(P, w)

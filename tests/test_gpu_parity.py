@@ -176,6 +176,39 @@ def test_fused_step_on_matrices_with_few_off_diagonal_values(P, s, values):
     assert np.all(np.abs(Y.cpu().numpy() - want) <= 1e-13 * (mag + 1e-300))
 
 
+@pytest.mark.parametrize("s", (1, 16))
+def test_ham_from_csr_ex_no_snapshot_sees_in_place_value_updates(P, s):
+    """a handle over a caller-owned CSR snapshots the values when they take one or two
+    off-diagonal values (packed form).  With POLFED_HAM_NO_SNAPSHOT it holds no copy: a step after an
+    in-place change of `val` must use the new values (the mapping is the caller's).
+    The handle is built on a side stream, the one the arrays were written on."""
+    n = 70_001                                    # above the persistent-filter sizes
+    rng = np.random.default_rng(77 + s)
+    cols = np.stack([(np.arange(n) + 1) % n, (np.arange(n) + n - 1) % n, np.arange(n)], axis=1)
+    cols.sort(axis=1)
+    vals = np.where(cols == np.arange(n)[:, None], rng.standard_normal((n, 3)), 0.5)   # one off-diagonal value
+    row_ptr = (3 * np.arange(n + 1)).astype(np.int32)
+    H = core.CSR(n, row_ptr, cols.reshape(-1).astype(np.int32), vals.reshape(-1).copy())
+    X = rng.standard_normal((n, s))
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        d_rp, d_col, d_val = dev(H.row_ptr), dev(H.col), dev(H.val)
+        ham = P.polfed_ham_from_csr_ex(d_rp, d_col, d_val, P.HAM_NO_SNAPSHOT)
+        Y = torch.full((n, s), float("nan"), dtype=torch.float64, device="cuda")
+        P.polfed_fused_step(ham, s, 1.0, 0.0, 0.0, 0.0, dev(X), None, None, Y)
+        first = Y.cpu().numpy()
+        H2 = core.CSR(n, H.row_ptr, H.col, H.val * np.where(H.col % 2 == 0, -3.0, 1.5))
+        d_val.copy_(torch.from_numpy(H2.val))     # in place: same device array
+        P.polfed_fused_step(ham, s, 1.0, 0.0, 0.0, 0.0, dev(X), None, None, Y)
+        second = Y.cpu().numpy()
+    for got, Hk in ((first, H), (second, H2)):
+        want = core.spmm(Hk, X)
+        mag = core.spmm(core.CSR(n, Hk.row_ptr, Hk.col, np.abs(Hk.val)), np.abs(X))
+        assert np.all(np.abs(got - want) <= 1e-13 * (mag + 1e-300))
+    with pytest.raises(P.PolfedError):
+        P.polfed_ham_from_csr_ex(d_rp, d_col, d_val, 2)          # unknown flag
+
+
 @pytest.mark.parametrize("n,s,K,avg", [(924, 1, 1000, 7), (1, 1, 5, 7), (300, 8, 385, 7), (513, 4, 384, 7),
                                        (4096, 1, 769, 7), (128, 32, 50, 7), (4097, 1, 40, 7),
                                        # rows of at most 16 entries and n * s <= 1024: entries in registers

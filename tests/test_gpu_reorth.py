@@ -37,6 +37,28 @@ def test_block_gram_and_update_match_numpy(P, n, k, s, variant):
     assert np.max(np.abs(dB.cpu().numpy() - want_B)) <= 1e-12 * np.abs(want_B).max()
 
 
+def test_block_products_reject_misaligned_and_overlapping_blocks(P):
+    """the header promises 16-byte aligned pointers; the tensor-core update moves B in
+    16-byte pieces, so an 8-byte aligned B must come back as POLFED_EINVAL, not as a device fault."""
+    import ctypes as C
+    n, s, k = 64, 16, 2
+    buf = torch.zeros(k * n * s + n * s + k * s * s + 8, dtype=torch.float64, device="cuda")
+    q, b, c = buf.data_ptr(), buf.data_ptr() + 8 * k * n * s, buf.data_ptr() + 8 * (k + 1) * n * s
+    L, vp = P.lib(), C.c_void_p
+    ok = lambda rc: rc == 0
+    assert ok(L.polfed_block_gram(s, n, vp(q), k, n * s, vp(b), vp(c), 0, None))
+    assert ok(L.polfed_block_update(s, n, vp(q), k, n * s, vp(c), -1.0, 1.0, vp(b), None))
+    for args in ((q + 8, b, c), (q, b + 8, c), (q, b, c + 8)):
+        assert L.polfed_block_gram(s, n, vp(args[0]), k, n * s, vp(args[1]), vp(args[2]), 0, None) == 1
+        assert L.polfed_block_gram_static(s, n, vp(args[0]), k, n * s, vp(args[1]), vp(args[2]), 0, None) == 1
+        assert L.polfed_block_update(s, n, vp(args[0]), k, n * s, vp(args[2]), -1.0, 1.0, vp(args[1]), None) == 1
+    # overlapping panels
+    assert L.polfed_block_gram(s, n, vp(q), k, n * s - 2, vp(b), vp(c), 0, None) == 1
+    assert L.polfed_block_update(s, n, vp(q), k, n * s - 2, vp(c), -1.0, 1.0, vp(b), None) == 1
+    torch.cuda.synchronize()                      # and the context is still healthy
+    assert float(buf.sum()) == 0.0
+
+
 @pytest.mark.parametrize("variant", (0, 1, 2))
 def test_block_gram_is_bit_reproducible(P, variant):
     gen = torch.Generator(device="cuda").manual_seed(7)
