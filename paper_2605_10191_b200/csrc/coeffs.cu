@@ -10,9 +10,16 @@ namespace {
 
 // T_n(lambda) for n = 0..K by the three-term recurrence Eq. (28)-(30), re-anchored on the
 // cosine form every 64 terms so rounding does not accumulate over long orders.
+// At lambda = 0 (the middle of the spectrum, where every mid-spectrum solve sits) the values are
+// known exactly: T_n(0) = cos(n pi/2) = 0 for odd n, (-1)^(n/2) for even n.  cos(n * acos(0)) would
+// give ~1e-16 instead of 0 there, and a non-zero c_n costs the fused step its V read (R22).
 void chebyshev_at(double lam, int K, std::vector<double>& T) {
   T.assign((size_t)K + 1, 1.0);
   if (K == 0) return;
+  if (lam == 0.0) {
+    for (int n = 1; n <= K; ++n) T[n] = (n & 1) ? 0.0 : ((n & 2) ? -1.0 : 1.0);
+    return;
+  }
   const double theta = std::acos(lam);
   T[1] = lam;
   for (int n = 2; n <= K; ++n) {

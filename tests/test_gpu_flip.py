@@ -98,6 +98,26 @@ def test_flip_filter_matches_oracle(P, L_outer, K):
     assert rel_l2(W.cpu().numpy(), want) <= 1e-9
 
 
+def test_flip_filter_with_the_librarys_exact_zero_coefficients(P):
+    """R22 / VERDICT r2: target in the middle of the interval (lambda~ = 0), the library's
+    coefficients (odd ones exactly 0, Eq. 33) on both sides: the flip steps without a V read."""
+    w = workloads.make_workload(4, L_override=9)
+    _, H = core.hamiltonian(w)
+    v0 = workloads.start_block(H.n, 1, seed=3004)[:, 0]
+    _, _, a, b = lanczos.spectrum_bounds(H, v0, m=60, margin=0.01)
+    K = 640
+    coeffs = P.polfed_filter_coeffs(a, b, a, K_in=K)
+    assert np.count_nonzero(coeffs[1::2]) == 0 and np.count_nonzero(coeffs[0::2]) == K // 2 + 1
+    V = workloads.start_block(H.n, w.s, seed=2004, orthonormal=True)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    ham = build(P, w.n_sites, w.terms, w.dot_bits, w.dot_dense)
+    W = torch.empty(H.n, w.s, dtype=torch.float64, device="cuda")
+    work = torch.empty(P.polfed_filter_workspace_bytes_ham(ham, w.s) // 8, dtype=torch.float64,
+                       device="cuda")
+    P.polfed_filter_apply(ham, a, b, coeffs, w.s, dev(V), W, work)
+    assert rel_l2(W.cpu().numpy(), want) <= 1e-9
+
+
 def test_flip_eigensolver_and_small_block_sizes(P):
     """The eigen-solver on a flip handle (every fused step goes through the flip kernel) returns
     true eigenpairs; block sizes the flip kernel does not cover use the CSR of the same handle."""

@@ -332,6 +332,24 @@ def test_filter_matches_oracle_on_workloads(P, config, L_override, K):
     assert np.linalg.norm(got) < np.linalg.norm(V)
 
 
+@pytest.mark.parametrize("config,L_override,K", [(2, None, 700), (3, 18, 640)])
+def test_filter_with_the_librarys_exact_zero_coefficients(P, config, L_override, K):
+    """R22 / VERDICT r2: at lambda~ = 0 the library's odd coefficients are exactly 0 (Eq. 33,
+    T_n(0) = 0) and every second launch skips its V read.  The oracle's own coefficients never hit
+    that path (cos(n pi/2) ~ 6e-17), so here BOTH sides get the library's coefficients: the persistent
+    small-matrix kernel (config 2) and the single-launch CSR / packed step (config 3 at L = 18)."""
+    w = workloads.make_workload(config, L_override=L_override)
+    _, H = core.hamiltonian(w)
+    a, b, _, _, _ = bounds_and_coeffs(w, H, K)
+    coeffs = P.polfed_filter_coeffs(a, b, a, K_in=K)
+    assert np.count_nonzero(coeffs[1::2]) == 0 and np.count_nonzero(coeffs[0::2]) == K // 2 + 1
+    V = workloads.start_block(H.n, w.s, seed=2000 + config, orthonormal=True)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    basis = P.polfed_build_basis(w.n_sites, w.n_up)
+    ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense)
+    assert rel_l2(run_filter(P, ham, a, b, coeffs, V), want) <= 1e-9
+
+
 def test_filter_host_entry_point_equals_device_entry_point(P):
     w = workloads.make_workload(2)
     _, H = core.hamiltonian(w)

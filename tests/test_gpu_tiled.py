@@ -97,6 +97,24 @@ def test_tiled_filter_matches_oracle_on_workloads(P, config, L_override, K, fmt)
     assert K <= 5000 and rel_l2(got, want) <= 1e-9
 
 
+@pytest.mark.parametrize("fmt", FORMATS)
+@pytest.mark.parametrize("config,L_override,K", [(5, 16, 640), (3, 14, 641)])
+def test_tiled_filter_with_the_librarys_exact_zero_coefficients(P, config, L_override, K, fmt):
+    """R22 / VERDICT r2: the sweeps without a V read (odd c_k exactly 0 at lambda~ = 0, Eq. 33),
+    judged by the oracle at depth: both sides get the library's coefficients."""
+    w = workloads.make_workload(config, L_override=L_override)
+    _, H = core.hamiltonian(w)
+    from oracle import lanczos
+    v0 = workloads.start_block(H.n, 1, seed=3000 + config)[:, 0]
+    _, _, a, b = lanczos.spectrum_bounds(H, v0, m=60, margin=0.01)
+    coeffs = P.polfed_filter_coeffs(a, b, a, K_in=K)
+    assert np.count_nonzero(coeffs[1::2]) == 0 and np.count_nonzero(coeffs[0::2]) == K // 2 + 1
+    V = workloads.start_block(H.n, w.s, seed=2000 + config, orthonormal=True)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    got = tiled_filter(P, build(P, w.n_sites, w.n_up, w.terms, fmt), a, b, coeffs, V)
+    assert rel_l2(got, want) <= 1e-9
+
+
 def test_tiled_handles_signs_long_hops_and_several_amplitudes(P):
     """Negative amplitudes, a hop across the cut, duplicate bonds, periodic closure, four
     distinct |amp| inside a tile."""

@@ -66,6 +66,22 @@ def test_filter_coeffs_match_oracle(lib, lam, K):
     assert abs(cheb.filter_value(got, [lam])[0] - 1.0) < 1e-12
 
 
+def test_filter_coeffs_at_mid_spectrum_have_exact_zeros(lib):
+    """Eq. (33): c_n is proportional to T_n(lambda~), and T_n(0) = 0 exactly for odd
+    n.  The library must return exact zeros there at every order (R22: a zero coefficient lets the
+    fused step skip its V read) -- K = 13 422 is config 3's order -- and +-2/chi at the even ones."""
+    a, b, K = -0.7, 2.5, 13422
+    got = P.polfed_filter_coeffs(a, b, a, K_in=K)           # sigma = a: lambda~ = 0 exactly
+    assert np.count_nonzero(got[1::2]) == 0 and got[1::2].size == 6711
+    chi = 1.0 + 2.0 * (K // 2)                               # 1 + 2 * #(even n in 1..K)
+    n_even = np.arange(2, K + 1, 2)
+    assert got[0] == 1.0 / chi
+    assert np.array_equal(got[2::2], np.where(n_even % 4 == 0, 2.0, -2.0) / chi)
+    want = cheb.filter_coeffs(0.0, K)
+    eps = np.finfo(np.float64).eps
+    assert np.max(np.abs(got - want)) <= (4 + 4 * K) * eps * np.max(np.abs(want))
+
+
 @pytest.mark.parametrize("lam,nev,rho", [(0.0, 50, 20000.0), (0.1, 50, 20000.0),
                                          (-0.3, 20, 900.0), (0.45, 100, 3.0e5)])
 def test_order_rule_matches_oracle(lib, lam, nev, rho):
