@@ -179,3 +179,32 @@ def test_flip_full_size_config4_sampled_rows(P):
     Y2 = torch.empty_like(B1)
     P.polfed_fused_step(csr, s, 2.0 / b, -2.0 * a / b, -1.0, ck, B1, B2, V, Y2)
     assert float((Y - Y2).norm() / Y2.norm()) <= 1e-14
+
+
+def test_flip_full_size_config4_filter_K1000_whole_block_against_oracle(P):
+    """Config 4 at full size (quantum sun, D = 2^20, s = 16), K = 1000 (SURVEY 8(d)'s K_par), every
+    element judged by the ORACLE: its CSR of the whole matrix, its textbook Clenshaw (Eq. 51
+    PAPER.md:427-431) on the whole block, against polfed_filter_apply on the flip handle (the path
+    bench.py times) and on the CSR handle.  rel l2 <= 1e-9 (north_star)."""
+    w = workloads.make_workload(4)
+    _, H = core.hamiltonian(w)
+    n, s, K = H.n, w.s, 1000
+    assert n == 1 << 20 and H.nnz == 26_214_400
+    v0 = workloads.start_block(n, 1, seed=3004)[:, 0]
+    _, _, a, b = lanczos.spectrum_bounds(H, v0, m=60, margin=0.01)
+    lam = (w.target - a) / b
+    coeffs = cheb.filter_coeffs(lam, K)
+    V = workloads.start_block(n, s, seed=2004, orthonormal=True)
+    want = core.clenshaw(H, a, b, coeffs, V)
+    del H
+    basis = P.polfed_build_basis(w.n_sites, w.n_up)
+    for fmt in (P.FORMAT_FLIP, P.FORMAT_CSR):
+        ham = P.polfed_build_hamiltonian(basis, w.terms, w.dot_bits, w.dot_dense, fmt=fmt)
+        W = torch.full((n, s), float("nan"), dtype=torch.float64, device="cuda")
+        work = torch.empty(P.polfed_filter_workspace_bytes_ham(ham, s) // 8, dtype=torch.float64,
+                           device="cuda")
+        P.polfed_filter_apply(ham, a, b, coeffs, s, dev(V), W, work)
+        got = W.cpu().numpy()
+        assert np.all(np.isfinite(got)), fmt
+        assert rel_l2(got, want) <= 1e-9, fmt
+        assert np.max(np.abs(got - want)) <= 1e-11 * np.abs(want).max(), fmt
