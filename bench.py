@@ -523,6 +523,7 @@ def hot_path_on_config(P, config: int, peak: float, fmt_name: str = ""):
             # the same byte count over the time of one product inside polfed_filter_apply (for the
             # small configs the single launches above are bound by the Python call, not the GPU)
             "frac_of_measured_in_filter": by / (apply_ms * 1e-3 / K) / 1e9 / peak,
+            "traffic": recorded_traffic(WORKLOAD_NAMES[config] + "/" + fmt_name),
             "l2": "inputs exceed L2" if by > 4 * 126e6 else "working set fits L2 (not flushed)"}
 
 

@@ -3,7 +3,7 @@
 // entries become one 32-bit word, column | value class << 28; the diagonal is a dense array.  A
 // stored entry then costs 4 bytes of stream instead of 12 and ONE quad shuffle in the fused
 // kernel instead of three (the kernel is bound by the LSU pipe that shuffles share with the
-// gathers, profiles/r01_flip_config4.md).  Built for every handle whose matrix qualifies
+// gathers, profiles/r03_flip_config4.md).  Built for every handle whose matrix qualifies
 // (dimension below 2^28, one or two off-diagonal values: XXZ chains); the kernels are in
 // spmm_clenshaw.cu.
 #include <cub/cub.cuh>
