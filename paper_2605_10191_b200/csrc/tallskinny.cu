@@ -8,7 +8,8 @@
 // factors and with them the iteration count of the eigen-solver are reproducible run to run.
 // For s in {8, 16, 32} the Gram product runs on the fp64 tensor cores (mma.sync m8n8k4, operands
 // straight from global memory into fragments); the shared-memory FMA kernel serves s < 8 and is
-// the measured alternative (profiles/r02_reorth.md).
+// the measured alternative (profiles/r02_reorth.md); with 4 panels or more one warp takes one panel and
+// the warps of a CTA share the rows of B through L1 (gram_dmma_panels_kernel, profiles/r03_gram_panels.md).
 #include <mutex>
 
 #include "common.cuh"
@@ -139,6 +140,65 @@ gram_dmma_kernel(long long n, const double* __restrict__ Q, size_t panel_stride,
     for (int w = 0; w < WARPS; ++w) t += red[w][o];
     partial[((size_t)blockIdx.x * gridDim.y + j) * OUT + o] = t;
   }
+}
+
+// The same product for several panels at once, W read once per CTA (round 3; with one
+// panel per CTA the rows of B were fetched once per panel, 1.6 x the algorithmic DRAM traffic at 8
+// panels).  The four warps of a CTA take four DIFFERENT panels and walk the SAME row groups, so the
+// 64-byte row pieces of B that the first warp brings into L1 serve the other three; each warp owns
+// its panel's accumulators, so there is no reduction inside the CTA: partial sum (x, j) is written
+// straight from the fragments.  Row group g -> CTA column (g mod gridDim.x), ascending: fixed order.
+template <int S>
+__global__ void __launch_bounds__(kDmmaThreads)
+gram_dmma_panels_kernel(long long n, const double* __restrict__ Q, int n_panels, size_t panel_stride,
+                        const double* __restrict__ B, double* __restrict__ partial) {
+  constexpr int T = S / 8, OUT = S * S, WARPS = kDmmaThreads / 32;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int j = blockIdx.y * WARPS + warp;
+  if (j >= n_panels) return;
+  const double* Qj = Q + (size_t)j * panel_stride + (lane & 3) * S + (lane >> 2);
+  const double* Bl = B + (lane & 3) * S + (lane >> 2);
+  double acc[T][T][2];
+#pragma unroll
+  for (int m = 0; m < T; ++m)
+#pragma unroll
+    for (int c = 0; c < T; ++c) acc[m][c][0] = acc[m][c][1] = 0.0;
+  const long long groups = n / 4;
+  for (long long g = blockIdx.x; g < groups; g += gridDim.x) {
+    const size_t at = (size_t)g * 4 * S;
+    double a[T], b[T];
+#pragma unroll
+    for (int m = 0; m < T; ++m) {
+      a[m] = __ldg(Qj + at + m * 8);
+      b[m] = __ldg(Bl + at + m * 8);
+    }
+#pragma unroll
+    for (int m = 0; m < T; ++m)
+#pragma unroll
+      for (int c = 0; c < T; ++c) dmma(acc[m][c][0], acc[m][c][1], a[m], b[c]);
+  }
+  if (blockIdx.x == 0 && groups * 4 < n) {  // the last n mod 4 rows: missing rows feed zeros
+    const size_t at = (size_t)groups * 4 * S;
+    const bool ok = groups * 4 + (lane & 3) < n;
+    double a[T], b[T];
+#pragma unroll
+    for (int m = 0; m < T; ++m) {
+      a[m] = ok ? __ldg(Qj + at + m * 8) : 0.0;
+      b[m] = ok ? __ldg(Bl + at + m * 8) : 0.0;
+    }
+#pragma unroll
+    for (int m = 0; m < T; ++m)
+#pragma unroll
+      for (int c = 0; c < T; ++c) dmma(acc[m][c][0], acc[m][c][1], a[m], b[c]);
+  }
+  double* out = partial + ((size_t)blockIdx.x * n_panels + j) * OUT;
+#pragma unroll
+  for (int m = 0; m < T; ++m)
+#pragma unroll
+    for (int c = 0; c < T; ++c) {
+      const int row = m * 8 + (lane >> 2), col = c * 8 + 2 * (lane & 3);
+      *reinterpret_cast<double2*>(out + row * S + col) = make_double2(acc[m][c][0], acc[m][c][1]);
+    }
 }
 
 // out[i] = sum over p = 0..count-1 (ascending) of partial[p * len + i]
@@ -343,6 +403,26 @@ int gram_launch(long long n, const double* Q, int n_panels, size_t stride, const
                 int sm_count, int variant, cudaStream_t st) {
   const bool dmma_ok = S >= 8;
   const bool use_dmma = dmma_ok && variant != 1;
+  if constexpr (S >= 8) {
+    if (use_dmma && n_panels >= 4) {  // one warp per panel, B read once per CTA
+      constexpr int WARPS = kDmmaThreads / 32;
+      const int gy = (n_panels + WARPS - 1) / WARPS;
+      int occ = 0;
+      POLFED_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, gram_dmma_panels_kernel<S>,
+                                                                kDmmaThreads, 0));
+      const long long groups = n / 4;
+      long long gxp = (long long)sm_count * (occ > 0 ? occ : 4) / gy;  // one wave of resident CTAs
+      if (gxp > groups) gxp = groups;
+      if (gxp < 1) gxp = 1;
+      const size_t lenp = (size_t)n_panels * S * S;
+      PoolBuf part(st);
+      POLFED_CUDA(part.alloc((size_t)gxp * lenp));
+      gram_dmma_panels_kernel<S><<<dim3((unsigned)gxp, (unsigned)gy), kDmmaThreads, 0, st>>>(
+          n, Q, n_panels, stride, B, part.p);
+      POLFED_LAUNCH_CHECK("gram_dmma_panels_kernel");
+      return sum_partials((int)gxp, lenp, part.p, C, st);
+    }
+  }
   long long gx;
   if (use_dmma) {
     const long long groups = (n / 4 + kDmmaThreads / 32 - 1) / (kDmmaThreads / 32);

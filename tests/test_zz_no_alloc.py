@@ -6,7 +6,7 @@ synchronisation.  Its partial sums sit in one 4 MiB array inside the library ins
 Checked here: on two calls in a row (the second smaller than the first and with another block size,
 so that the array still holds the first call's partial sums when the second runs) the result agrees
 with polfed_block_gram on the same inputs within the bound tests/test_gpu_reorth.py uses against
-numpy, and bit for bit where both paths take the same grid; a panel list beyond the stated limit is
+numpy, and bit for bit where both paths run the same kernel on the same grid; a panel list beyond the stated limit is
 refused before anything is launched.
 
 The file name sorts last on purpose: `pytest -x` stops at the first failure, and a failure here must
@@ -57,8 +57,11 @@ def test_static_gram_matches_the_pool_path_on_two_calls_in_a_row(P, variant):
     for (k, n, s), out, ref in zip(CALLS, outs, want):
         err = (out - ref).abs().max().item()
         assert np.isfinite(err) and err <= _bound(n), (k, n, s, err)
-    # same grid on both paths (8 CTAs per SM fit the array at s = 16): the sums are bit-identical
-    assert torch.equal(outs[1], want[1])
+    # the shared-memory FMA kernel takes the same grid on both paths at s = 16 (8 CTAs per SM fit the
+    # array): bit-identical sums.  (variant 0 is the tensor-core kernel, which on the pool path walks
+    # several panels per CTA and so adds in another order.)
+    if variant == 1:
+        assert torch.equal(outs[1], want[1])
     # and against numpy, so that the check does not rest on the pool path alone
     Q, B = inputs[1]
     exact = np.einsum("jra,rb->jab", Q.cpu().numpy(), B.cpu().numpy())
