@@ -601,6 +601,7 @@ def time_to_nev(P, config: int, window_levels: int = 0):
             "seconds": wall, "seconds_inside_library": rep["seconds_total"], "window_levels": rep["nev_window"],
             "converged": rep["status"] == 0, "K": rep["K"], "block_steps": rep["block_steps"],
             "krylov_dim": rep["krylov_dim"], "sparse_products": rep["sparse_products"],
+            "fraction_of_products_without_v_read": rep["products_without_v"] / max(rep["sparse_products"], 1),
             "max_residual_over_normH": float(resid.max()) / hnorm,
             "seconds_filter": rep["seconds_filter"], "seconds_reorth": rep["seconds_reorth"],
             "seconds_qr": rep["seconds_qr"], "seconds_projected_eig": rep["seconds_projected_eig"],

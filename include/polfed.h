@@ -384,6 +384,9 @@ typedef struct {
   int32_t nev_window;             /* levels the filter window is sized for: nev + max(2, 10 %), or
                                      options->window_levels */
   double seconds_dos;             /* moments of the density-of-states estimate */
+  int64_t products_without_v;     /* of sparse_products: filter launches whose coefficient is exactly 0 and
+                                     that therefore skip the read of V (R22; about half of them when the
+                                     target is the middle of the interval) */
 } polfed_report;
 
 /* The nev eigenpairs of H nearest sigma (Sec. 4.6 steps 1-6):

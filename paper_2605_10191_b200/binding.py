@@ -68,7 +68,7 @@ class _Report(C.Structure):
                 ("seconds_projected_eig", C.c_double), ("seconds_extraction", C.c_double),
                 ("seconds_total", C.c_double), ("rho_gaussian", C.c_double),
                 ("rho_kpm", C.c_double), ("K_kpm", C.c_int32), ("nev_window", C.c_int32),
-                ("seconds_dos", C.c_double)]
+                ("seconds_dos", C.c_double), ("products_without_v", C.c_int64)]
 
 
 _lib = None

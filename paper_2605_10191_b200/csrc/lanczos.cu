@@ -431,6 +431,9 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
   rc = qr.twice(Q, Bk.data());
   if (rc) return rc;
 
+  // launches of one filter application that skip V: steps k = K-1 .. 0 with c_k == 0 exactly (R22)
+  long long zero_coeffs = 0;
+  for (int kk = 0; kk < K; ++kk) zero_coeffs += coeffs[kk] == 0.0 ? 1 : 0;
   int next_check = (wp + s - 1) / s;
   int status = POLFED_ENOCONV;
   int k = 0;
@@ -444,6 +447,7 @@ int polfed_block_lanczos_eigs(const polfed_ham* ham, double sigma, int nev, int 
     POLFED_CUDA(cudaStreamSynchronize(st));
     rep.seconds_filter += now_seconds() - t0;
     rep.sparse_products += K;
+    rep.products_without_v += zero_coeffs;
 
     // A_k = V_k^T W and full reorthogonalisation against V_1..V_k, twice (Eq. 9, 11)
     t0 = now_seconds();

@@ -97,6 +97,9 @@ def test_eigs_config2_full_pipeline_matches_dense(P):
         assert np.min(np.abs(ev - lam_)) <= 1e-9 * hnorm
     assert rep["sparse_products"] >= rep["K"] * rep["block_steps"]
     assert rep["seconds_filter"] > 0 and rep["seconds_total"] >= rep["seconds_filter"]
+    # R22: at lambda~ = 0 the odd coefficients are exact zeros at every order, so the launches of the
+    # odd steps k = 1, 3, .. <= K-1 skip the V read
+    assert rep["products_without_v"] == (rep["K"] // 2) * rep["block_steps"]
 
 
 @pytest.mark.parametrize("config,L_override,nev", [(4, 9, 24), (5, 14, 40), (3, 14, 30)])
